@@ -1,0 +1,258 @@
+#!/usr/bin/env python
+"""bench.py -- fp64 cell-updates/s of the whole hot path (one "step" = S(dt/2) + sweep + sweep + S(dt/2) + CFL)
+on BASELINE.json's synthetic cavity fields, one process per GPU.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C5] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `value` = cells * steps * ranks / max-over-ranks device time with the state
+resident in HBM; `e2e` = the same metric through the C ABI with HOST buffers (initial state uploaded from
+pinned host memory, K steps, diagnostics and all 7 fields read back), copies inside the timed region;
+`roofline` = the dominant kernel (directional sweep) against the FP64-ALU peak;
+`cpu_baseline` = the oracle timed on this box's host cores on a bounded crop of the same workload.
+The path does not shard (single-GPU method): --gpus N runs N independent replicas ("replicas only").
+`--impl reference` times the oracle (tests' CPU implementation) instead of the CUDA path.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1905_05727_b200 import inputs  # noqa: E402
+
+METRIC = "fp64 cell-updates/s per 2D step"
+UNIT = "cell-updates/s"
+# algorithmic FP64 work of one cell-step (two sweeps + two source half-steps + CFL),
+# counted on the oracle's arithmetic with the CUDA math-library expansions of div/sqrt/exp/log
+FLOP_PER_CELL_SWEEP = 1560.0      # one directional sweep of one cell (dadd+dmul = 1, dfma = 2)
+FP64_LANES_PER_SM, N_SM = 64, 148
+
+
+def peaks():
+    p = {}
+    try:
+        p = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    return p
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)"""
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) >= 7:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_rate(cfg_name, budget_s=12.0, crop=(2048, 512)):
+    """the oracle as it stands on a bounded crop of the workload; returns (cell-updates/s, cores, sample text)"""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle_py as O
+    cores = os.cpu_count() or 1
+    cfg = inputs.config(cfg_name, nx=crop[0], ny=crop[1])
+    o = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=cores)
+    o.init(cfg["init"])
+    t0 = time.perf_counter()
+    o.step(1)
+    t1 = time.perf_counter() - t0
+    n = max(1, min(50, int(budget_s / max(t1, 1e-3))))
+    t0 = time.perf_counter()
+    o.step(n)
+    el = time.perf_counter() - t0
+    cells = crop[0] * crop[1]
+    return cells * n / el, cores, "%s crop %dx%d, %d steps (%.1f s), OpenMP over rows, %d threads" % (
+        cfg_name, crop[0], crop[1], n, el, cores), el / n
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, args.steps)
+    crop = (1024, 256)
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle_py as O
+    cores = os.cpu_count() or 1
+    cfg = inputs.config(args.config, nx=crop[0], ny=crop[1])
+    o = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=cores)
+    o.init(cfg["init"])
+    o.step(max(0, min(args.warmup, 3)))
+    t0 = time.perf_counter()
+    o.step(steps)
+    el = time.perf_counter() - t0
+    v = crop[0] * crop[1] * steps / el
+    sample = "%s crop %dx%d per step (oracle, OpenMP over rows, %d threads)" % (args.config, crop[0], crop[1], cores)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": el / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s (%s)" % (args.config, sample)},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C5")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--variant", type=int, default=1)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1905_05727_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    K, Wm = max(1, args.steps), max(3, args.warmup)
+
+    cfg = inputs.config(args.config, seed=inputs.config(args.config)["init"]["seed"] + rank if args.config in ("C4", "C5") else None)
+    g = cfg["grid"]
+    cells = g["nx"] * g["ny"]
+    sim = binding.Sim(g, cfg["eos"], cfg["kin"], variant=args.variant)
+    sim.init(cfg["init"])
+    ncav = len(sim.cavities())
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------------------
+    sim.step(Wm)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = sim.launch_count()
+    sim.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(sim.stream)
+    sim.step(K)
+    e1.record(sim.stream)
+    barrier()
+    sim.profile(False)
+    launches = sim.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    kt = sim.kernel_times()
+    d = sim.diagnostics()
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = cells * K * world / (ms * 1e-3)
+
+    # ---- roofline of the dominant kernel --------------------------------------------------------------------
+    pk = peaks()
+    clk = sampler.summary()
+    sm_max = pk.get("sm_max_mhz", clk.get("sm_max_mhz") or 1965.0)
+    peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    dom = max(("sweep_x", "sweep_y"), key=lambda k: kt[k][0])
+    dom_ms = kt[dom][0] / max(kt[dom][1], 1)
+    achieved = FLOP_PER_CELL_SWEEP * cells / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+            "frac": achieved / peak_tflops, "traffic": None, "peak_source": "148 SM x 64 FP64 lanes x 2 x sm_max_mhz (nominal)",
+            "ms_per_launch": dom_ms,
+            "hbm_gbs_algorithmic": 112.0 * cells / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0,
+            "hbm_peak_gbs": pk.get("hbm_gbs", 6650.0),
+            "kernel_ms_per_step": {k: v[0] / K for k, v in kt.items()}}
+
+    # ---- end to end through the C ABI with host buffers -------------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        host = [torch.empty((g["ny"], g["nx"]), dtype=torch.float64).pin_memory() for _ in range(7)]
+        views = [h.numpy() for h in host]
+        for k in range(7):
+            sim.read_field_into(k, views[k])
+        sim.init(cfg["init"])                      # fresh initial state for the e2e job
+        for k in range(7):
+            sim.read_field_into(k, views[k])
+        barrier()
+        t0 = time.perf_counter()
+        sim.init_fields_ptr(views)                 # H2D of the step inputs (7 planes from pinned host memory)
+        sim.step(K)
+        de = sim.diagnostics()                     # D2H of the job's metric
+        for k in range(7):
+            sim.read_field_into(k, views[k])       # D2H of the result fields
+        barrier()
+        el = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([el], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        nbytes = 7 * cells * 8
+        e2e = {"value": cells * K * world / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
+               "job": "sim_init_fields(host) + sim_step(%d) + sim_diagnostics + 7 x sim_read_field(host)" % K, "seconds": el,
+               "M2r": de["M2r"]}
+
+    if rank != 0:
+        return
+    cpu = None
+    if not args.no_cpu and world == 1:
+        v, cores, sample, _ = oracle_rate(args.config)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s %dx%d, %d cavities, p_shock %.3g Pa, fp64 SoA 7 planes double-buffered; replicas only; "
+                               "state %.1f MB > L2 (no flush needed)" % (args.config, g["nx"], g["ny"], ncav, cfg["init"]["p_shock"],
+                                                                          7 * cells * 8 / 1e6),
+                   "variant": args.variant, "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
+        "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+        "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "burned_mass": d["burned_mass"]},
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

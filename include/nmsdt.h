@@ -1,0 +1,154 @@
+/*
+ * nmsdt.h -- C ABI of libnmsdt.so: the B200 (sm_100a) hot path of Mi et al., arXiv:1905.05727,
+ * "Meso-resolved simulations of shock-to-detonation transition in nitromethane with air-filled cavities".
+ *
+ * What the library computes: the per-time-step finite-volume update of the 2D diffuse-interface two-fluid
+ * (air cavities = phase 1, liquid nitromethane = phase 2) reactive Euler equations, Eq. 1,
+ * with the Cochran-Chan / ideal-gas equations of state Eq. 2-5, single-step Arrhenius kinetics Eq. 6
+ * (P:114), MUSCL-Hancock + slope limiter + HLLC with Strang splitting, in fp64, entirely in CUDA
+ * kernels on one GPU.  Points the paper leaves open are fixed by the readings R1..R22 of DESIGN.md.
+ *
+ * Conventions
+ *  - plain C; every call returns 0 on success or a negative code:
+ *      SIM_ERR_ARG (-1) bad argument, SIM_ERR_CUDA (-2) CUDA runtime error, SIM_ERR_STATE (-3) not initialised,
+ *      SIM_ERR_BAD (-4) non-finite or non-positive state detected on the device.
+ *    sim_last_error() returns a static / handle-owned string describing the last failure.
+ *  - pointers named host_* / *_out are HOST pointers owned by the caller; the library never keeps them.
+ *    `device_buf` is a DEVICE pointer.  No exception crosses the ABI.
+ *  - all work is enqueued on the stream given to sim_create; calls marked [sync] block on that stream,
+ *    calls marked [async] return immediately (the time step dt lives in device memory, so sim_step(n)
+ *    never synchronises with the host).
+ *  - there is no CPU fallback: without a CUDA device sim_create fails with SIM_ERR_CUDA.
+ *
+ * State per cell (SoA, fp64, 7 planes), Eq. 1:
+ *   q0 = z1 rho1, q1 = z2 rho2, q2 = rho u, q3 = rho v, q4 = rho E, q5 = z1, q6 = z2 rho2 lambda
+ * lambda = mass fraction of UNREACTED nitromethane, 1 -> 0.
+ * Device layout: each plane is (ny+4) rows of `pitch` doubles, pitch = roundup(16 + nx + 2, 16); interior
+ * cell (i,j) sits at row j+2, column 16+i, so that every interior row starts 128-byte aligned; two ghost
+ * rows/columns on each side are filled by the halo step.  Two such sets of 7 planes (ping-pong) plus small
+ * reduction scratch make up the workspace (sim_workspace_bytes).
+ */
+#ifndef NMSDT_H
+#define NMSDT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sim sim_t;
+
+enum { SIM_OK = 0, SIM_ERR_ARG = -1, SIM_ERR_CUDA = -2, SIM_ERR_STATE = -3, SIM_ERR_BAD = -4 };
+/* boundary kinds (P:129 inflow/transmissive left, P:135 periodic top/bottom; R12) */
+enum { SIM_BC_TRANSMISSIVE = 0, SIM_BC_PERIODIC = 1, SIM_BC_REFLECTIVE = 2, SIM_BC_INFLOW_FIXED = 3 };
+/* slope limiter ("van Leer non-smooth slope limiter"; R5): minmod form (default) or monotonised central */
+enum { SIM_LIM_MINMOD = 0, SIM_LIM_MC = 1 };
+/* field ids for sim_read_field */
+enum { SIM_F_Q0 = 0, SIM_F_Q1, SIM_F_Q2, SIM_F_Q3, SIM_F_Q4, SIM_F_Q5, SIM_F_Q6,
+       SIM_F_P = 16, SIM_F_T2 = 17, SIM_F_RHO = 18, SIM_F_U = 19, SIM_F_V = 20, SIM_F_LAMBDA = 21,
+       SIM_F_PROGRESS = 22 /* 1 - lambda */, SIM_F_RHO2 = 23, SIM_F_C = 24, SIM_F_T1 = 25, SIM_F_RHO1 = 26 };
+/* kernel variants (sim_set_variant): 0 = unfused reference kernels (halo, source, sweep, CFL as separate
+   launches), 1 = fused production path (default). Both compute the same step. */
+enum { SIM_VARIANT_UNFUSED = 0, SIM_VARIANT_FUSED = 1 };
+
+typedef struct {
+    int nx, ny;                 /* interior cells */
+    double dx, dy;              /* metres */
+    int bc_xlo, bc_xhi, bc_ylo, bc_yhi;
+    double cfl;                 /* R11: dt = cfl * min(dx,dy) / max(max(|u|,|v|) + c) */
+    int limiter;                /* SIM_LIM_* */
+} sim_grid_t;
+
+/* Table I, Table II, T_ref,2 = 0 K; z_min clamps the volume fractions */
+typedef struct {
+    double gamma1, cv1;
+    double Gamma2, A, B, C, D, rho02, cv2, Tref2;
+    double z_min;
+} sim_eos_t;
+
+/* Table III.  RK4 sub-stepping rule R13: n_sub = min(max_substeps, 1 + floor(theta/substep_theta)) */
+typedef struct {
+    double Ta, Cpre, Q;
+    int reactive;               /* 0: inert (source step skipped) */
+    int max_substeps;
+    double substep_theta;
+} sim_kin_t;
+
+typedef struct { double x, y, r; } sim_cavity_t;   /* centre and radius in cell units */
+
+/* problem setup.  Cavities come from exactly one of: explicit list (ncav > 0), square lattice
+   (lattice != 0; Eq. 7 geometry), or the seeded generator (phi > 0; Eq. 8, R16). */
+typedef struct {
+    double p_shock;             /* input shock pressure [Pa]; slab i < shock_cells is set to the neat-NM Hugoniot state */
+    int shock_cells;            /* L_s in cells */
+    double p0, rho1_0, rho2_0;  /* ambient state */
+    double interface_width;     /* tanh interface width in cells; h = width/2 (R15) */
+    const sim_cavity_t* cav; int ncav;              /* HOST pointer, copied during the call */
+    unsigned long long seed; double phi, dmin, dmax, min_gap; int x_lo, x_hi;
+    int lattice; double lattice_d, lattice_spacing;
+} sim_init_t;
+
+typedef struct {
+    double t; long long step; double dt_last, smax;
+    double M2r, M2tot0, burned_mass, rate_inst;     /* Eq. 12-13 */
+    double mass1, mass2, momx, momy, energy;        /* integrals of q0..q4 */
+    int bad_state;
+} sim_diag_t;
+
+/* Bytes of device memory sim_create needs for this grid (0 on bad argument). Host-only computation. */
+size_t sim_workspace_bytes(const sim_grid_t* grid);
+
+/* Create a simulation. device_buf: DEVICE pointer to >= sim_workspace_bytes() bytes, 256-byte aligned, lent by
+   the caller for the lifetime of the handle (e.g. a torch tensor), or NULL to let the library cudaMalloc it.
+   cuda_stream: a cudaStream_t (NULL = default stream). [sync] */
+int sim_create(const sim_grid_t* grid, const sim_eos_t* eos, const sim_kin_t* kin,
+               void* device_buf, size_t bytes, void* cuda_stream, sim_t** out);
+void sim_destroy(sim_t*);
+const char* sim_last_error(const sim_t*);          /* sim may be NULL: error of the last failed sim_create */
+
+/* Initial condition on the device: cavity placement (generator R16 runs on the GPU), tanh painting,
+   ambient state and shocked slab (O7).  Resets t, step; computes M2,tot and the first CFL dt. [sync] */
+int sim_init(sim_t*, const sim_init_t*);
+/* Explicit initial state from 7 HOST arrays of nx*ny doubles (row-major, x fastest). [sync] */
+int sim_init_fields(sim_t*, const double* const host_q[7]);
+
+/* CFL time step of the current state (a7). [sync] */
+int sim_cfl_dt(sim_t*, double* dt_out);
+/* n CFL-limited steps (O6: S(dt/2) X Y S(dt/2) on even steps, S Y X S on odd steps). [async] */
+int sim_step(sim_t*, int n);
+/* n steps with the given fixed dt (parity tests). [async] */
+int sim_step_dt(sim_t*, int n, double dt);
+/* Pieces of the step, exposed for parity tests: halo fill for a sweep direction (0 = x, 1 = y), one
+   directional sweep (halo + MUSCL-Hancock/HLLC update), the source step over tau on every cell. [async] */
+int sim_halo(sim_t*, int dir);
+int sim_sweep(sim_t*, int dir, double dt);
+int sim_source(sim_t*, double tau);
+
+/* Global diagnostics (a8): Eq. 12 reactive mass, conservation integrals, instantaneous rate, S_max. [sync] */
+int sim_diagnostics(sim_t*, sim_diag_t* out);
+/* Copy one field (SIM_F_*) to host_out[nx*ny], row-major, x fastest. [sync] */
+int sim_read_field(sim_t*, int field_id, double* host_out);
+/* Cavity list used by the last sim_init (generator parity). Writes min(n, cap) entries. [sync] */
+int sim_get_cavities(sim_t*, sim_cavity_t* host_out, int cap, int* n);
+
+/* Select kernel variant (SIM_VARIANT_*) and whether sim_step replays CUDA graphs (default on). */
+int sim_set_variant(sim_t*, int variant, int use_graph);
+/* Number of kernel launches enqueued by this handle so far (bench.py's gpu_launches). */
+long long sim_launch_count(const sim_t*);
+/* Device pointer / layout of plane k of the current state (for zero-copy consumers). */
+int sim_device_layout(const sim_t*, void** plane0, long long* plane_stride, int* pitch, int* x_offset, int* y_offset);
+/* Per-kernel device timing with CUDA events on the handle's stream (bench.py's roofline block).
+   sim_profile(s, 1) starts recording an event pair around every step kernel (graphs are bypassed while on);
+   sim_profile(s, 0) stops and resolves them [sync]; sim_kernel_time returns the accumulated milliseconds and
+   launch count of one kernel kind (SIM_K_*) since the last sim_profile(s, 1). */
+enum { SIM_K_SWEEP_X = 0, SIM_K_SWEEP_Y = 1, SIM_K_SOURCE = 2, SIM_K_CFL = 3, SIM_K_HALO = 4, SIM_K_NKIND = 5 };
+int sim_profile(sim_t*, int on);
+int sim_kernel_time(const sim_t*, int kind, double* ms_total, long long* launches);
+/* Measured FP64 FMA throughput of this device in GFLOP/s (2 flop per DFMA), probe kernel of ~ms. [sync] */
+int sim_probe_fp64(sim_t*, double* gflops_out, double* ms_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -430,7 +430,7 @@ extern "C" int orc_init(orc_t* s, const orc_init_t* in)
                 if (per_y && ddy > 0.5 * ny) ddy = ny - ddy;     /* minimum image */
                 double d = std::sqrt(ddx * ddx + ddy * ddy);
                 double sarg = (d - c.r) / h;
-                double val = sarg >= 20.0 ? 0.0 : 0.5 * (1.0 - std::tanh(sarg));
+                double val = sarg >= 20.0 ? 0.0 : 1.0 / (1.0 + std::exp(2.0 * sarg));   /* = 1/2 [1 - tanh(s)], well conditioned in the tail */
                 double& pr = prof[(size_t)j * nx + i];
                 if (val > pr) pr = val;
             }

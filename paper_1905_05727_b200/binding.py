@@ -1,0 +1,267 @@
+"""Thin ctypes binding of libnmsdt.so (include/nmsdt.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; PyTorch is used for device memory
+(the workspace is a torch uint8 tensor lent to sim_create) and for the CUDA stream.  There is no CPU
+fallback: importing works anywhere (so that symbol checks can run without a GPU), but creating a `Sim`
+without the built library or without a CUDA device raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libnmsdt.so")
+
+SIM_OK, SIM_ERR_ARG, SIM_ERR_CUDA, SIM_ERR_STATE, SIM_ERR_BAD = 0, -1, -2, -3, -4
+VARIANT_UNFUSED, VARIANT_FUSED = 0, 1
+FIELD = {"q0": 0, "q1": 1, "q2": 2, "q3": 3, "q4": 4, "q5": 5, "q6": 6, "p": 16, "T2": 17, "rho": 18, "u": 19,
+         "v": 20, "lambda": 21, "progress": 22, "rho2": 23, "c": 24, "T1": 25, "rho1": 26}
+
+# every symbol include/nmsdt.h declares (tests check that the library exports each one)
+SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error", "sim_init", "sim_init_fields",
+           "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
+           "sim_read_field", "sim_get_cavities", "sim_set_variant", "sim_launch_count", "sim_device_layout",
+           "sim_probe_fp64", "sim_profile", "sim_kernel_time"]
+KERNEL_KINDS = {"sweep_x": 0, "sweep_y": 1, "source": 2, "cfl": 3, "halo": 4}
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("dx", C.c_double), ("dy", C.c_double),
+                ("bc_xlo", C.c_int), ("bc_xhi", C.c_int), ("bc_ylo", C.c_int), ("bc_yhi", C.c_int),
+                ("cfl", C.c_double), ("limiter", C.c_int)]
+
+
+class Eos(C.Structure):
+    _fields_ = [(n, C.c_double) for n in
+                ("gamma1", "cv1", "Gamma2", "A", "B", "C", "D", "rho02", "cv2", "Tref2", "z_min")]
+
+
+class Kin(C.Structure):
+    _fields_ = [("Ta", C.c_double), ("Cpre", C.c_double), ("Q", C.c_double), ("reactive", C.c_int),
+                ("max_substeps", C.c_int), ("substep_theta", C.c_double)]
+
+
+class Cavity(C.Structure):
+    _fields_ = [("x", C.c_double), ("y", C.c_double), ("r", C.c_double)]
+
+
+class Init(C.Structure):
+    _fields_ = [("p_shock", C.c_double), ("shock_cells", C.c_int), ("p0", C.c_double), ("rho1_0", C.c_double),
+                ("rho2_0", C.c_double), ("interface_width", C.c_double), ("cav", C.POINTER(Cavity)),
+                ("ncav", C.c_int), ("seed", C.c_ulonglong), ("phi", C.c_double), ("dmin", C.c_double),
+                ("dmax", C.c_double), ("min_gap", C.c_double), ("x_lo", C.c_int), ("x_hi", C.c_int),
+                ("lattice", C.c_int), ("lattice_d", C.c_double), ("lattice_spacing", C.c_double)]
+
+
+class Diag(C.Structure):
+    _fields_ = [("t", C.c_double), ("step", C.c_longlong), ("dt_last", C.c_double), ("smax", C.c_double),
+                ("M2r", C.c_double), ("M2tot0", C.c_double), ("burned_mass", C.c_double), ("rate_inst", C.c_double),
+                ("mass1", C.c_double), ("mass2", C.c_double), ("momx", C.c_double), ("momy", C.c_double),
+                ("energy", C.c_double), ("bad_state", C.c_int)]
+
+
+class NmsdtError(RuntimeError):
+    def __init__(self, what, code, msg):
+        super().__init__("%s failed (%d): %s" % (what, code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """Load libnmsdt.so (no CUDA call is made). Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libnmsdt.so is not built: run `python -m paper_1905_05727_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    dp, vp = C.POINTER(C.c_double), C.c_void_p
+    sig = {
+        "sim_workspace_bytes": (C.c_size_t, [C.POINTER(Grid)]),
+        "sim_create": (C.c_int, [C.POINTER(Grid), C.POINTER(Eos), C.POINTER(Kin), vp, C.c_size_t, vp, C.POINTER(vp)]),
+        "sim_destroy": (None, [vp]),
+        "sim_last_error": (C.c_char_p, [vp]),
+        "sim_init": (C.c_int, [vp, C.POINTER(Init)]),
+        "sim_init_fields": (C.c_int, [vp, C.POINTER(dp)]),
+        "sim_cfl_dt": (C.c_int, [vp, dp]),
+        "sim_step": (C.c_int, [vp, C.c_int]),
+        "sim_step_dt": (C.c_int, [vp, C.c_int, C.c_double]),
+        "sim_halo": (C.c_int, [vp, C.c_int]),
+        "sim_sweep": (C.c_int, [vp, C.c_int, C.c_double]),
+        "sim_source": (C.c_int, [vp, C.c_double]),
+        "sim_diagnostics": (C.c_int, [vp, C.POINTER(Diag)]),
+        "sim_read_field": (C.c_int, [vp, C.c_int, dp]),
+        "sim_get_cavities": (C.c_int, [vp, C.POINTER(Cavity), C.c_int, C.POINTER(C.c_int)]),
+        "sim_set_variant": (C.c_int, [vp, C.c_int, C.c_int]),
+        "sim_launch_count": (C.c_longlong, [vp]),
+        "sim_device_layout": (C.c_int, [vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(C.c_int),
+                                        C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+        "sim_probe_fp64": (C.c_int, [vp, dp, dp]),
+        "sim_profile": (C.c_int, [vp, C.c_int]),
+        "sim_kernel_time": (C.c_int, [vp, C.c_int, dp, C.POINTER(C.c_longlong)]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _fill(struct, d):
+    for k, v in d.items():
+        setattr(struct, k, v)
+    return struct
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def workspace_bytes(grid):
+    return int(load_library().sim_workspace_bytes(C.byref(_fill(Grid(), grid))))
+
+
+class Sim:
+    """One simulation on the current CUDA device. grid/eos/kin/init are plain dicts (see `inputs`)."""
+
+    def __init__(self, grid, eos, kin, device=None, variant=None, use_graph=True):
+        import torch
+        self.L = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1905_05727_b200 needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device(device if device is not None else "cuda:%d" % torch.cuda.current_device())
+        self.grid = _fill(Grid(), grid)
+        self.eos = _fill(Eos(), eos)
+        self.kin = _fill(Kin(), kin)
+        self.nx, self.ny = self.grid.nx, self.grid.ny
+        nbytes = int(self.L.sim_workspace_bytes(C.byref(self.grid)))
+        if nbytes == 0:
+            raise NmsdtError("sim_workspace_bytes", SIM_ERR_ARG, "bad grid")
+        self.h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # device memory: torch's
+            self.stream = torch.cuda.current_stream(self.device)
+            rc = self.L.sim_create(C.byref(self.grid), C.byref(self.eos), C.byref(self.kin),
+                                   C.c_void_p(self.workspace.data_ptr()), nbytes, C.c_void_p(self.stream.cuda_stream),
+                                   C.byref(self.h))
+        if rc != 0:
+            raise NmsdtError("sim_create", rc, (self.L.sim_last_error(None) or b"").decode())
+        if variant is not None:
+            self.set_variant(variant, use_graph)
+
+    # -- plumbing ------------------------------------------------------------------------------------
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise NmsdtError(what, rc, (self.L.sim_last_error(self.h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.sim_destroy(self.h)
+            self.h = C.c_void_p()
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the calls of include/nmsdt.h ------------------------------------------------------------------
+    def init(self, init):
+        d = dict(init)
+        cav = d.pop("cavities", None)
+        ini = _fill(Init(), d)
+        keep = None
+        if cav is not None and len(cav) > 0:
+            keep = (Cavity * len(cav))(*[Cavity(float(c[0]), float(c[1]), float(c[2])) for c in cav])
+            ini.cav = C.cast(keep, C.POINTER(Cavity))
+            ini.ncav = len(cav)
+        self._chk(self.L.sim_init(self.h, C.byref(ini)), "sim_init")
+
+    def init_fields(self, q):
+        q = [np.ascontiguousarray(a, dtype=np.float64).reshape(self.ny, self.nx) for a in q]
+        ptrs = (C.POINTER(C.c_double) * 7)(*[_dp(a) for a in q])
+        self._chk(self.L.sim_init_fields(self.h, ptrs), "sim_init_fields")
+
+    def cfl_dt(self):
+        dt = C.c_double()
+        self._chk(self.L.sim_cfl_dt(self.h, C.byref(dt)), "sim_cfl_dt")
+        return dt.value
+
+    def step(self, n=1):
+        self._chk(self.L.sim_step(self.h, int(n)), "sim_step")
+
+    def step_dt(self, n, dt):
+        self._chk(self.L.sim_step_dt(self.h, int(n), float(dt)), "sim_step_dt")
+
+    def halo(self, d):
+        self._chk(self.L.sim_halo(self.h, int(d)), "sim_halo")
+
+    def sweep(self, d, dt):
+        self._chk(self.L.sim_sweep(self.h, int(d), float(dt)), "sim_sweep")
+
+    def source(self, tau):
+        self._chk(self.L.sim_source(self.h, float(tau)), "sim_source")
+
+    def diagnostics(self, allow_bad=False):
+        d = Diag()
+        rc = self.L.sim_diagnostics(self.h, C.byref(d))
+        if not (allow_bad and rc == SIM_ERR_BAD):
+            self._chk(rc, "sim_diagnostics")
+        return {n: getattr(d, n) for n, _ in Diag._fields_}
+
+    def read_field(self, fid):
+        if isinstance(fid, str):
+            fid = FIELD[fid]
+        out = np.empty((self.ny, self.nx), dtype=np.float64)
+        self._chk(self.L.sim_read_field(self.h, int(fid), _dp(out)), "sim_read_field")
+        return out
+
+    def state(self):
+        return [self.read_field(k) for k in range(7)]
+
+    def cavities(self):
+        n = C.c_int()
+        self._chk(self.L.sim_get_cavities(self.h, None, 0, C.byref(n)), "sim_get_cavities")
+        arr = (Cavity * max(n.value, 1))()
+        self._chk(self.L.sim_get_cavities(self.h, arr, n.value, C.byref(n)), "sim_get_cavities")
+        return np.array([[arr[i].x, arr[i].y, arr[i].r] for i in range(n.value)], dtype=np.float64).reshape(-1, 3)
+
+    def set_variant(self, variant, use_graph=True):
+        self._chk(self.L.sim_set_variant(self.h, int(variant), int(bool(use_graph))), "sim_set_variant")
+
+    def launch_count(self):
+        return int(self.L.sim_launch_count(self.h))
+
+    def probe_fp64(self):
+        g, ms = C.c_double(), C.c_double()
+        self._chk(self.L.sim_probe_fp64(self.h, C.byref(g), C.byref(ms)), "sim_probe_fp64")
+        return g.value, ms.value
+
+    def profile(self, on):
+        self._chk(self.L.sim_profile(self.h, int(bool(on))), "sim_profile")
+
+    def kernel_times(self):
+        """{kind: (total ms, launches)} accumulated between profile(True) and profile(False)"""
+        out = {}
+        for name, kid in KERNEL_KINDS.items():
+            ms, n = C.c_double(), C.c_longlong()
+            self._chk(self.L.sim_kernel_time(self.h, kid, C.byref(ms), C.byref(n)), "sim_kernel_time")
+            out[name] = (ms.value, int(n.value))
+        return out
+
+    def init_fields_ptr(self, arrays):
+        """arrays: 7 C-contiguous float64 numpy arrays (e.g. views of pinned torch tensors); no copy is made"""
+        ptrs = (C.POINTER(C.c_double) * 7)(*[_dp(a) for a in arrays])
+        self._chk(self.L.sim_init_fields(self.h, ptrs), "sim_init_fields")
+
+    def read_field_into(self, fid, out):
+        self._chk(self.L.sim_read_field(self.h, int(fid), _dp(out)), "sim_read_field")
+
+    def synchronize(self):
+        self.stream.synchronize()

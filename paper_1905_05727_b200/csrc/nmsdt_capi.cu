@@ -1,0 +1,485 @@
+// nmsdt_capi.cu -- the C ABI of libnmsdt.so (include/nmsdt.h): handle, workspace layout, step orchestration.
+#include "../../include/nmsdt.h"
+#include "nmsdt_host.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace nmsdt;
+
+namespace {
+
+std::string g_create_error;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    int pitch, rows;
+    long long fstride;       // doubles
+    size_t off_A, off_B, off_inflow, off_partial, off_diag, off_ctl, off_scratch, total;
+};
+
+Layout make_layout(int nx, int ny)
+{
+    Layout L;
+    L.pitch = (int)align_up((size_t)(NGX + nx + NG), 16);
+    L.rows = ny + 2 * NGY;
+    L.fstride = (long long)L.pitch * L.rows;
+    size_t plane_set = (size_t)7 * L.fstride * sizeof(double);
+    size_t o = 0;
+    L.off_A = o; o = align_up(o + plane_set, 256);
+    L.off_B = o; o = align_up(o + plane_set, 256);
+    L.off_inflow = o; o = align_up(o + (size_t)7 * ny * sizeof(double), 256);
+    L.off_partial = o; o = align_up(o + (size_t)DIAG_BLOCKS * (DIAG_NV + 1) * sizeof(double), 256);
+    L.off_diag = o; o = align_up(o + sizeof(DiagOut), 256);
+    L.off_ctl = o; o = align_up(o + sizeof(Ctl), 256);
+    L.off_scratch = o; o = align_up(o + 8 * sizeof(double), 256);
+    L.total = o;
+    return L;
+}
+
+} // namespace
+
+struct sim {
+    sim_grid_t g;
+    sim_eos_t e;
+    sim_kin_t k;
+    Params P;
+    Layout L;
+    cudaStream_t stream = nullptr;
+    char* base = nullptr;
+    bool owns = false;
+    double *A = nullptr, *B = nullptr, *inflow = nullptr, *partial = nullptr, *scratch = nullptr;
+    DiagOut* d_diag = nullptr;
+    Ctl* ctl = nullptr;
+    Cav* d_cav = nullptr;
+    int ncav = 0;
+    bool inited = false;
+    long long host_step = 0;        // mirrors ctl->step (step parity decides the sweep order)
+    double M2tot0 = 0.0;
+    int variant = SIM_VARIANT_UNFUSED;
+    int use_graph = 0;
+    long long launches = 0;
+    std::string err;
+    // event profiling (sim_profile)
+    struct EvPair { cudaEvent_t a, b; int kind; };
+    std::vector<EvPair> ev;
+    size_t ev_used = 0;
+    bool profile = false;
+    double kms[SIM_K_NKIND] = {0, 0, 0, 0, 0};
+    long long kcount[SIM_K_NKIND] = {0, 0, 0, 0, 0};
+};
+
+namespace {
+
+int fail(sim* s, int code, const std::string& msg)
+{
+    if (s) s->err = msg; else g_create_error = msg;
+    return code;
+}
+
+int check_cuda(sim* s, const char* what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(s, SIM_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    return SIM_OK;
+}
+
+bool grid_ok(const sim_grid_t* g)
+{
+    if (!g || g->nx < 1 || g->ny < 1 || !(g->dx > 0.0) || !(g->dy > 0.0) || !(g->cfl > 0.0)) return false;
+    const int b[4] = {g->bc_xlo, g->bc_xhi, g->bc_ylo, g->bc_yhi};
+    for (int i = 0; i < 4; ++i) if (b[i] < 0 || b[i] > 3) return false;
+    if (g->bc_xhi == SIM_BC_INFLOW_FIXED || g->bc_ylo == SIM_BC_INFLOW_FIXED || g->bc_yhi == SIM_BC_INFLOW_FIXED) return false;
+    if ((g->bc_xlo == SIM_BC_PERIODIC) != (g->bc_xhi == SIM_BC_PERIODIC)) return false;
+    if ((g->bc_ylo == SIM_BC_PERIODIC) != (g->bc_yhi == SIM_BC_PERIODIC)) return false;
+    if (g->limiter != SIM_LIM_MINMOD && g->limiter != SIM_LIM_MC) return false;
+    return true;
+}
+
+void fill_params(sim* s)
+{
+    Params& P = s->P;
+    const sim_grid_t& g = s->g; const sim_eos_t& e = s->e; const sim_kin_t& k = s->k;
+    P.nx = g.nx; P.ny = g.ny; P.pitch = s->L.pitch; P.rows = s->L.rows; P.fstride = s->L.fstride;
+    P.dx = g.dx; P.dy = g.dy; P.cfl = g.cfl; P.hmin = g.dx < g.dy ? g.dx : g.dy;
+    P.bc_xlo = g.bc_xlo; P.bc_xhi = g.bc_xhi; P.bc_ylo = g.bc_ylo; P.bc_yhi = g.bc_yhi; P.limiter = g.limiter;
+    P.gamma1 = e.gamma1; P.G1 = e.gamma1 - 1.0; P.iG1 = 1.0 / P.G1; P.cv1 = e.cv1;
+    P.G2 = e.Gamma2; P.iG2 = 1.0 / e.Gamma2; P.G2p1 = e.Gamma2 + 1.0;
+    P.A = e.A; P.B = e.B; P.C = e.C; P.D = e.D; P.rho02 = e.rho02; P.irho02 = 1.0 / e.rho02; P.cv2 = e.cv2; P.Tref2 = e.Tref2;
+    P.kA = -e.A / (1.0 - e.C); P.kB = e.B / (1.0 - e.D); P.AC = e.A * e.C; P.BD = e.B * e.D;
+    P.z_min = e.z_min; P.z_max = 1.0 - e.z_min;
+    P.Ta = k.Ta; P.Cpre = k.Cpre; P.Q = k.Q; P.theta0 = k.substep_theta; P.reactive = k.reactive; P.max_substeps = k.max_substeps;
+}
+
+// host-side scalar model functions for the Hugoniot root find (O7)
+double h_pref(const sim_eos_t& e, double rho) { double x = rho / e.rho02; return e.A * std::pow(x, e.C) - e.B * std::pow(x, e.D); }
+double h_eref(const sim_eos_t& e, double rho)
+{
+    double x = rho / e.rho02;
+    return -e.A / (e.rho02 * (1.0 - e.C)) * (std::pow(x, e.C - 1.0) - 1.0) + e.B / (e.rho02 * (1.0 - e.D)) * (std::pow(x, e.D - 1.0) - 1.0);
+}
+double h_e2(const sim_eos_t& e, double rho, double p) { return h_eref(e, rho) + (p - h_pref(e, rho)) / (rho * e.Gamma2); }
+
+bool hugoniot(const sim_eos_t& e, double p0, double rho1_0, double rho2_0, double ps, Hug& out)
+{
+    const double e0 = h_e2(e, rho2_0, p0), v0 = 1.0 / rho2_0;
+    auto f = [&](double rho) { return h_e2(e, rho, ps) - e0 - 0.5 * (ps + p0) * (v0 - 1.0 / rho); };
+    double lo = rho2_0 * (1.0 + 1e-12), hi = rho2_0 * 1.5;
+    if (!(ps > p0) || !(f(lo) > 0.0)) return false;
+    int guard = 0;
+    while (f(hi) > 0.0) { hi *= 1.5; if (++guard > 40) return false; }
+    for (int it = 0; it < 200; ++it) { double mid = 0.5 * (lo + hi); if (f(mid) > 0.0) lo = mid; else hi = mid; }
+    const double rs = 0.5 * (lo + hi);
+    out.rho_s = rs;
+    out.u_p = std::sqrt((ps - p0) * (v0 - 1.0 / rs));
+    out.U_s = out.u_p / (1.0 - rho2_0 / rs);
+    out.T2_s = e.Tref2 + (ps - h_pref(e, rs)) / (rs * e.Gamma2 * e.cv2);
+    const double g = e.gamma1;
+    out.rho1_s = rho1_0 * ((g + 1.0) * ps + (g - 1.0) * p0) / ((g - 1.0) * ps + (g + 1.0) * p0);
+    return true;
+}
+
+// event pair around one kernel launch while profiling
+struct KTimer {
+    sim* s; int idx = -1;
+    KTimer(sim* s_, int kind) : s(s_)
+    {
+        if (!s->profile) return;
+        if (s->ev_used == s->ev.size()) {
+            sim::EvPair p; cudaEventCreate(&p.a); cudaEventCreate(&p.b); p.kind = kind;
+            s->ev.push_back(p);
+        }
+        idx = (int)s->ev_used++;
+        s->ev[idx].kind = kind;
+        cudaEventRecord(s->ev[idx].a, s->stream);
+    }
+    ~KTimer() { if (idx >= 0) cudaEventRecord(s->ev[idx].b, s->stream); }
+};
+
+// one full step on the unfused reference path: CFL, S(dt/2), sweep, sweep, S(dt/2)
+void enqueue_step_unfused(sim* s)
+{
+    cudaStream_t st = s->stream;
+    const Params& P = s->P;
+    { KTimer t(s, SIM_K_CFL); launch_cfl(P, s->A, s->ctl, st); }
+    launch_finalize_dt(P, s->ctl, st);
+    s->launches += 2;
+    const double* dtp = &s->ctl->dt;
+    if (P.reactive) { KTimer t(s, SIM_K_SOURCE); launch_source(P, s->A, dtp, 0.5, st); s->launches++; }
+    const int d1 = (s->host_step & 1) ? 1 : 0, d2 = 1 - d1;
+    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->A, s->inflow, d1, st); }
+    { KTimer t(s, d1 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_march(P, s->A, s->B, dtp, d1, st); }
+    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->B, s->inflow, d2, st); }
+    { KTimer t(s, d2 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_march(P, s->B, s->A, dtp, d2, st); }
+    s->launches += 4;
+    if (P.reactive) { KTimer t(s, SIM_K_SOURCE); launch_source(P, s->A, dtp, 0.5, st); s->launches++; }
+    launch_advance(s->ctl, st);
+    s->launches++;
+    s->host_step++;
+}
+
+int finish_init(sim* s)
+{
+    cudaStream_t st = s->stream;
+    launch_capture_inflow(s->P, s->A, s->inflow, st);
+    Ctl h; std::memset(&h, 0, sizeof(h));
+    cudaMemcpyAsync(s->ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, st);
+    cudaStreamSynchronize(st);
+    s->host_step = 0;
+    s->inited = true;
+    s->launches += 1;
+    sim_diag_t d;
+    s->M2tot0 = 0.0;
+    int rc = sim_diagnostics(s, &d);
+    if (rc != SIM_OK && rc != SIM_ERR_BAD) return rc;
+    s->M2tot0 = d.M2r;
+    return check_cuda(s, "init");
+}
+
+} // namespace
+
+extern "C" {
+
+size_t sim_workspace_bytes(const sim_grid_t* g)
+{
+    if (!grid_ok(g)) return 0;
+    return make_layout(g->nx, g->ny).total;
+}
+
+const char* sim_last_error(const sim_t* s) { return s ? s->err.c_str() : g_create_error.c_str(); }
+
+int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void* device_buf, size_t bytes, void* cuda_stream, sim_t** out)
+{
+    if (!out) return fail(nullptr, SIM_ERR_ARG, "sim_create: out is NULL");
+    *out = nullptr;
+    if (!grid_ok(g) || !e || !k) return fail(nullptr, SIM_ERR_ARG, "sim_create: bad grid / eos / kin argument");
+    if (!(e->z_min > 0.0 && e->z_min < 0.5) || !(e->gamma1 > 1.0) || !(e->Gamma2 > 0.0) || !(e->rho02 > 0.0) || e->C == 1.0 || e->D == 1.0)
+        return fail(nullptr, SIM_ERR_ARG, "sim_create: bad EOS parameters");
+    if (k->max_substeps < 1 || !(k->substep_theta > 0.0)) return fail(nullptr, SIM_ERR_ARG, "sim_create: bad kinetics parameters");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, SIM_ERR_CUDA, "sim_create: no CUDA device (libnmsdt has no CPU fallback)");
+    }
+    sim* s = new sim();
+    s->g = *g; s->e = *e; s->k = *k;
+    s->L = make_layout(g->nx, g->ny);
+    s->stream = (cudaStream_t)cuda_stream;
+    if (device_buf) {
+        if (bytes < s->L.total || ((uintptr_t)device_buf & 255)) { delete s; return fail(nullptr, SIM_ERR_ARG, "sim_create: device_buf too small or not 256-byte aligned"); }
+        s->base = (char*)device_buf;
+    } else {
+        if (cudaMalloc(&s->base, s->L.total) != cudaSuccess) { cudaGetLastError(); delete s; return fail(nullptr, SIM_ERR_CUDA, "sim_create: cudaMalloc failed"); }
+        s->owns = true;
+    }
+    s->A = (double*)(s->base + s->L.off_A); s->B = (double*)(s->base + s->L.off_B);
+    s->inflow = (double*)(s->base + s->L.off_inflow); s->partial = (double*)(s->base + s->L.off_partial);
+    s->d_diag = (DiagOut*)(s->base + s->L.off_diag); s->ctl = (Ctl*)(s->base + s->L.off_ctl);
+    s->scratch = (double*)(s->base + s->L.off_scratch);
+    fill_params(s);
+    cudaMemsetAsync(s->base, 0, s->L.total, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) { int rc = check_cuda(nullptr, "sim_create"); sim_destroy(s); return rc ? rc : SIM_ERR_CUDA; }
+    *out = s;
+    return SIM_OK;
+}
+
+void sim_destroy(sim_t* s)
+{
+    if (!s) return;
+    cudaStreamSynchronize(s->stream);
+    if (s->d_cav) cudaFree(s->d_cav);
+    for (auto& p : s->ev) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+    if (s->owns && s->base) cudaFree(s->base);
+    delete s;
+}
+
+int sim_init(sim_t* s, const sim_init_t* in)
+{
+    if (!s || !in) return fail(s, SIM_ERR_ARG, "sim_init: NULL argument");
+    if (in->shock_cells < 0 || in->shock_cells > s->g.nx || !(in->interface_width > 0.0)) return fail(s, SIM_ERR_ARG, "sim_init: bad shock_cells / interface_width");
+    cudaStream_t st = s->stream;
+    const Params& P = s->P;
+    if (s->d_cav) { cudaFree(s->d_cav); s->d_cav = nullptr; }
+    s->ncav = 0;
+    std::vector<Cav> host;
+    if (in->cav && in->ncav > 0) {
+        for (int i = 0; i < in->ncav; ++i) host.push_back({in->cav[i].x, in->cav[i].y, in->cav[i].r});
+    } else if (in->lattice) {     // R20: centres x_lo + s/2 + s i, s/2 + s j
+        if (!(in->lattice_spacing > 0.0) || !(in->lattice_d > 0.0)) return fail(s, SIM_ERR_ARG, "sim_init: bad lattice");
+        const double sp = in->lattice_spacing, r = 0.5 * in->lattice_d;
+        for (int jj = 0; sp * (jj + 1) <= (double)s->g.ny; ++jj)
+            for (int ii = 0; in->x_lo + sp * (ii + 1) <= (double)in->x_hi; ++ii) host.push_back({in->x_lo + 0.5 * sp + sp * ii, 0.5 * sp + sp * jj, r});
+    } else if (in->phi > 0.0) {
+        int n = generate_cavities(in->seed, in->phi, in->dmin, in->dmax, in->min_gap, in->x_lo, in->x_hi, s->g.ny,
+                                  s->g.bc_ylo == SIM_BC_PERIODIC ? 1 : 0, &s->d_cav, st, &s->launches);
+        if (n == -1) return fail(s, SIM_ERR_ARG, "sim_init: bad generator parameters");
+        if (n < 0) { cudaGetLastError(); return fail(s, SIM_ERR_CUDA, "sim_init: cavity generator failed"); }
+        s->ncav = n;
+    }
+    if (!host.empty()) {
+        if (cudaMalloc(&s->d_cav, sizeof(Cav) * host.size()) != cudaSuccess) { cudaGetLastError(); return fail(s, SIM_ERR_CUDA, "sim_init: cudaMalloc"); }
+        cudaMemcpyAsync(s->d_cav, host.data(), sizeof(Cav) * host.size(), cudaMemcpyHostToDevice, st);
+        cudaStreamSynchronize(st);
+        s->ncav = (int)host.size();
+    }
+    Hug hug = {0, 0, 0, 0, 0};
+    if (in->shock_cells > 0 && !hugoniot(s->e, in->p0, in->rho1_0, in->rho2_0, in->p_shock, hug)) return fail(s, SIM_ERR_ARG, "sim_init: Hugoniot solve failed");
+    launch_zero_plane(P, s->A + 5 * P.fstride, st);
+    launch_paint(P, s->A + 5 * P.fstride, s->d_cav, s->ncav, 0.5 * in->interface_width, st);
+    launch_fill_state(P, s->A, in->shock_cells, hug, in->p_shock, in->p0, in->rho1_0, in->rho2_0, st);
+    s->launches += 3;
+    return finish_init(s);
+}
+
+int sim_init_fields(sim_t* s, const double* const host_q[7])
+{
+    if (!s || !host_q) return fail(s, SIM_ERR_ARG, "sim_init_fields: NULL argument");
+    const Params& P = s->P;
+    for (int f = 0; f < 7; ++f) {
+        if (!host_q[f]) return fail(s, SIM_ERR_ARG, "sim_init_fields: NULL plane");
+        double* dst = s->A + f * P.fstride + (long long)NGY * P.pitch + NGX;
+        if (cudaMemcpy2DAsync(dst, (size_t)P.pitch * 8, host_q[f], (size_t)P.nx * 8, (size_t)P.nx * 8, P.ny, cudaMemcpyHostToDevice, s->stream) != cudaSuccess)
+            return check_cuda(s, "sim_init_fields");
+    }
+    cudaStreamSynchronize(s->stream);
+    if (s->d_cav) { cudaFree(s->d_cav); s->d_cav = nullptr; }
+    s->ncav = 0;
+    return finish_init(s);
+}
+
+int sim_cfl_dt(sim_t* s, double* dt_out)
+{
+    if (!s || !dt_out) return fail(s, SIM_ERR_ARG, "sim_cfl_dt: NULL argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_cfl_dt: not initialised");
+    launch_set_double(&s->ctl->dt_fixed, 0.0, s->stream);
+    launch_cfl(s->P, s->A, s->ctl, s->stream);
+    launch_finalize_dt(s->P, s->ctl, s->stream);
+    s->launches += 3;
+    Ctl h;
+    cudaMemcpyAsync(&h, s->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_cfl_dt");
+    *dt_out = h.dt;
+    if (h.bad) return fail(s, SIM_ERR_BAD, "sim_cfl_dt: non-finite or non-positive state");
+    return SIM_OK;
+}
+
+static int step_common(sim_t* s, int n, double dt_fixed)
+{
+    if (!s || n < 0) return fail(s, SIM_ERR_ARG, "sim_step: bad argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_step: not initialised");
+    launch_set_double(&s->ctl->dt_fixed, dt_fixed, s->stream);
+    s->launches++;
+    for (int it = 0; it < n; ++it) enqueue_step_unfused(s);
+    return check_cuda(s, "sim_step");
+}
+
+int sim_step(sim_t* s, int n) { return step_common(s, n, 0.0); }
+
+int sim_step_dt(sim_t* s, int n, double dt)
+{
+    if (!(dt > 0.0)) return fail(s, SIM_ERR_ARG, "sim_step_dt: dt must be positive");
+    return step_common(s, n, dt);
+}
+
+int sim_halo(sim_t* s, int dir)
+{
+    if (!s || (dir != 0 && dir != 1)) return fail(s, SIM_ERR_ARG, "sim_halo: bad argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_halo: not initialised");
+    launch_halo(s->P, s->A, s->inflow, dir, s->stream);
+    s->launches++;
+    return check_cuda(s, "sim_halo");
+}
+
+int sim_sweep(sim_t* s, int dir, double dt)
+{
+    if (!s || (dir != 0 && dir != 1) || !(dt > 0.0)) return fail(s, SIM_ERR_ARG, "sim_sweep: bad argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_sweep: not initialised");
+    launch_set_double(s->scratch, dt, s->stream);
+    launch_halo(s->P, s->A, s->inflow, dir, s->stream);
+    launch_sweep_march(s->P, s->A, s->B, s->scratch, dir, s->stream);
+    s->launches += 3;
+    // keep the state in A: copy the interior planes back (parity-test helper, not on the hot path)
+    cudaMemcpyAsync(s->A, s->B, (size_t)7 * s->P.fstride * sizeof(double), cudaMemcpyDeviceToDevice, s->stream);
+    return check_cuda(s, "sim_sweep");
+}
+
+int sim_source(sim_t* s, double tau)
+{
+    if (!s || !(tau > 0.0)) return fail(s, SIM_ERR_ARG, "sim_source: bad argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_source: not initialised");
+    if (!s->P.reactive) return SIM_OK;
+    launch_set_double(s->scratch, tau, s->stream);
+    launch_source(s->P, s->A, s->scratch, 1.0, s->stream);
+    s->launches += 2;
+    return check_cuda(s, "sim_source");
+}
+
+int sim_diagnostics(sim_t* s, sim_diag_t* out)
+{
+    if (!s || !out) return fail(s, SIM_ERR_ARG, "sim_diagnostics: NULL argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_diagnostics: not initialised");
+    launch_diag(s->P, s->A, s->partial, s->d_diag, s->stream);
+    s->launches += 2;
+    DiagOut d; Ctl c;
+    cudaMemcpyAsync(&d, s->d_diag, sizeof(DiagOut), cudaMemcpyDeviceToHost, s->stream);
+    cudaMemcpyAsync(&c, s->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_diagnostics");
+    const double dA = s->g.dx * s->g.dy;
+    out->t = c.t; out->step = c.step; out->dt_last = c.dt_last; out->smax = d.smax;
+    out->M2r = d.sum[5] * dA; out->M2tot0 = s->M2tot0; out->burned_mass = s->M2tot0 - out->M2r; out->rate_inst = d.sum[6] * dA;
+    out->mass1 = d.sum[0] * dA; out->mass2 = d.sum[1] * dA; out->momx = d.sum[2] * dA; out->momy = d.sum[3] * dA; out->energy = d.sum[4] * dA;
+    out->bad_state = (d.bad || c.bad) ? 1 : 0;
+    if (out->bad_state) return fail(s, SIM_ERR_BAD, "sim_diagnostics: non-finite or non-positive state");
+    return check_cuda(s, "sim_diagnostics");
+}
+
+int sim_read_field(sim_t* s, int fid, double* host_out)
+{
+    if (!s || !host_out) return fail(s, SIM_ERR_ARG, "sim_read_field: NULL argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_read_field: not initialised");
+    const Params& P = s->P;
+    if (fid >= 0 && fid < 7) {
+        const double* src = s->A + fid * P.fstride + (long long)NGY * P.pitch + NGX;
+        cudaMemcpy2DAsync(host_out, (size_t)P.nx * 8, src, (size_t)P.pitch * 8, (size_t)P.nx * 8, P.ny, cudaMemcpyDeviceToHost, s->stream);
+    } else if (fid >= 16 && fid <= 26) {
+        double* dense = s->B;    // B is free between steps
+        launch_derived(P, s->A, fid, dense, s->stream);
+        s->launches++;
+        cudaMemcpyAsync(host_out, dense, (size_t)P.nx * P.ny * 8, cudaMemcpyDeviceToHost, s->stream);
+    } else return fail(s, SIM_ERR_ARG, "sim_read_field: unknown field id");
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_read_field");
+    return check_cuda(s, "sim_read_field");
+}
+
+int sim_get_cavities(sim_t* s, sim_cavity_t* host_out, int cap, int* n)
+{
+    if (!s || !n) return fail(s, SIM_ERR_ARG, "sim_get_cavities: NULL argument");
+    *n = s->ncav;
+    const int m = s->ncav < cap ? s->ncav : cap;
+    if (m > 0 && host_out) {
+        static_assert(sizeof(sim_cavity_t) == sizeof(Cav), "cavity layout");
+        cudaMemcpyAsync(host_out, s->d_cav, sizeof(Cav) * (size_t)m, cudaMemcpyDeviceToHost, s->stream);
+        if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_get_cavities");
+    }
+    return SIM_OK;
+}
+
+int sim_set_variant(sim_t* s, int variant, int use_graph)
+{
+    if (!s || (variant != SIM_VARIANT_UNFUSED && variant != SIM_VARIANT_FUSED)) return fail(s, SIM_ERR_ARG, "sim_set_variant: bad argument");
+    s->variant = variant; s->use_graph = use_graph ? 1 : 0;
+    return SIM_OK;
+}
+
+long long sim_launch_count(const sim_t* s) { return s ? s->launches : 0; }
+
+int sim_device_layout(const sim_t* s, void** plane0, long long* plane_stride, int* pitch, int* x_offset, int* y_offset)
+{
+    if (!s) return SIM_ERR_ARG;
+    if (plane0) *plane0 = s->A;
+    if (plane_stride) *plane_stride = s->P.fstride;
+    if (pitch) *pitch = s->P.pitch;
+    if (x_offset) *x_offset = NGX;
+    if (y_offset) *y_offset = NGY;
+    return SIM_OK;
+}
+
+int sim_profile(sim_t* s, int on)
+{
+    if (!s) return SIM_ERR_ARG;
+    if (on) {
+        for (int k = 0; k < SIM_K_NKIND; ++k) { s->kms[k] = 0.0; s->kcount[k] = 0; }
+        s->ev_used = 0;
+        s->profile = true;
+        return SIM_OK;
+    }
+    s->profile = false;
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_profile");
+    for (size_t i = 0; i < s->ev_used; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, s->ev[i].a, s->ev[i].b) == cudaSuccess) { s->kms[s->ev[i].kind] += ms; s->kcount[s->ev[i].kind]++; }
+    }
+    s->ev_used = 0;
+    return check_cuda(s, "sim_profile");
+}
+
+int sim_kernel_time(const sim_t* s, int kind, double* ms_total, long long* launches)
+{
+    if (!s || kind < 0 || kind >= SIM_K_NKIND || !ms_total || !launches) return SIM_ERR_ARG;
+    *ms_total = s->kms[kind]; *launches = s->kcount[kind];
+    return SIM_OK;
+}
+
+int sim_probe_fp64(sim_t* s, double* gflops_out, double* ms_out)
+{
+    if (!s || !gflops_out || !ms_out) return fail(s, SIM_ERR_ARG, "sim_probe_fp64: NULL argument");
+    int rc = launch_probe_fp64(s->stream, gflops_out, ms_out);
+    if (rc) return fail(s, SIM_ERR_CUDA, "sim_probe_fp64 failed");
+    return SIM_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,44 @@
+// nmsdt_host.h -- host-side declarations shared by the .cu files of libnmsdt.so (not part of the public ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include "nmsdt_device.cuh"
+
+namespace nmsdt {
+
+struct Cav { double x, y, r; };
+
+struct Hug { double rho_s, U_s, u_p, T2_s, rho1_s; };
+
+struct DiagOut {   // device-side result of the diagnostics reduction
+    double sum[7]; // q0..q4, q6, rate
+    double smax;
+    int bad;
+    int pad;
+};
+
+constexpr int DIAG_BLOCKS = 1184;          // 8 x 148
+constexpr int DIAG_NV = 8;                 // 7 sums + smax
+
+// step kernels (nmsdt_step.cu)
+void launch_halo(const Params& P, double* q, const double* inflow, int dir, cudaStream_t s);
+void launch_source(const Params& P, double* q, const double* dtp, double scale, cudaStream_t s);
+void launch_sweep_march(const Params& P, const double* qin, double* qout, const double* dtp, int dir, cudaStream_t s);
+void launch_cfl(const Params& P, const double* q, Ctl* ctl, cudaStream_t s);
+void launch_finalize_dt(const Params& P, Ctl* ctl, cudaStream_t s);
+void launch_advance(Ctl* ctl, cudaStream_t s);
+void launch_set_double(double* p, double v, cudaStream_t s);
+int  launch_probe_fp64(cudaStream_t s, double* gflops, double* ms);
+
+// init / output kernels (nmsdt_init.cu)
+void launch_zero_plane(const Params& P, double* plane, cudaStream_t s);
+void launch_paint(const Params& P, double* prof_plane, const Cav* cav, int ncav, double h, cudaStream_t s);
+void launch_fill_state(const Params& P, double* q, int shock_cells, Hug hug, double p_shock, double p0, double rho1_0,
+                       double rho2_0, cudaStream_t s);
+void launch_capture_inflow(const Params& P, const double* q, double* inflow, cudaStream_t s);
+void launch_diag(const Params& P, const double* q, double* partial, DiagOut* out, cudaStream_t s);
+void launch_derived(const Params& P, const double* q, int field_id, double* out_dense, cudaStream_t s);
+// seeded generator on the device; returns number of cavities (<0 on error); list left in d_cav
+int  generate_cavities(unsigned long long seed, double phi, double dmin, double dmax, double min_gap, int x_lo, int x_hi,
+                       int ny, int periodic_y, Cav** d_cav_out, cudaStream_t s, long long* launches);
+
+} // namespace nmsdt

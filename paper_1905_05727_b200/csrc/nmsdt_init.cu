@@ -1,0 +1,383 @@
+// nmsdt_init.cu -- problem setup (a9: seeded cavity generator, tanh painting, shocked slab),
+// diagnostics reduction (a8; Eq. 12-13) and derived output fields of libnmsdt.so.
+#include "nmsdt_host.h"
+#include <cmath>
+#include <vector>
+
+namespace nmsdt {
+
+// ---------------------------------------------------------------------------------------------------------
+// painting: prof = max_k 1/2 [1 - tanh((d_k - R_k)/h)], exactly 0 beyond 20 h (R15).  One block per cavity;
+// non-negative doubles order like their bit patterns, so atomicMax on the bits is an exact max.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void k_zero_plane(const __grid_constant__ Params P, double* __restrict__ plane)
+{
+    const long long n = (long long)P.pitch * P.rows;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) plane[t] = 0.0;
+}
+void launch_zero_plane(const Params& P, double* plane, cudaStream_t s) { k_zero_plane<<<148 * 4, 256, 0, s>>>(P, plane); }
+
+__global__ void k_paint(const __grid_constant__ Params P, double* __restrict__ prof, const Cav* __restrict__ cav, int ncav, double h)
+{
+    const int k = blockIdx.x;
+    if (k >= ncav) return;
+    const Cav c = cav[k];
+    const bool per_y = P.bc_ylo == 1;
+    const double reach = c.r + 20.0 * h + 1.0;
+    const int i0 = max((int)floor(c.x - reach), 0), i1 = min((int)ceil(c.x + reach), P.nx - 1);
+    const int j0 = (int)floor(c.y - reach), j1 = (int)ceil(c.y + reach);
+    const int w = i1 - i0 + 1, hh = j1 - j0 + 1;
+    if (w <= 0) return;
+    for (int t = threadIdx.x; t < w * hh; t += blockDim.x) {
+        const int jj = j0 + t / w, i = i0 + t % w;
+        int j = jj;
+        if (per_y) j = ((jj % P.ny) + P.ny) % P.ny;
+        else if (jj < 0 || jj >= P.ny) continue;
+        const double ddx = (i + 0.5) - c.x;
+        double ddy = fabs((j + 0.5) - c.y);
+        if (per_y && ddy > 0.5 * P.ny) ddy = P.ny - ddy;            // minimum image
+        const double d = sqrt(ddx * ddx + ddy * ddy);
+        const double sarg = (d - c.r) / h;
+        const double val = sarg >= 20.0 ? 0.0 : 1.0 / (1.0 + exp(2.0 * sarg));      // = 1/2 [1 - tanh(s)]
+        if (val > 0.0)
+            atomicMax(reinterpret_cast<unsigned long long*>(prof + (long long)(j + NGY) * P.pitch + NGX + i), dbits(val));
+    }
+}
+void launch_paint(const Params& P, double* prof, const Cav* cav, int ncav, double h, cudaStream_t s)
+{
+    if (ncav > 0) k_paint<<<ncav, 256, 0, s>>>(P, prof, cav, ncav, h);
+}
+
+// ambient state / shocked slab; the painted profile sits in plane 5 on entry
+__global__ void k_fill_state(const __grid_constant__ Params P, double* __restrict__ q, int shock_cells, Hug hug, double p_shock,
+                             double p0, double rho1_0, double rho2_0)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (i >= P.nx) return;
+    const long long id = (long long)(j + NGY) * P.pitch + NGX + i;
+    double W[7];
+    if (i < shock_cells) {
+        W[0] = hug.rho1_s; W[1] = hug.rho_s; W[2] = hug.u_p; W[3] = 0.0; W[4] = p_shock; W[5] = P.z_min; W[6] = 0.0;
+    } else {
+        const double prof = q[5 * P.fstride + id];
+        W[0] = rho1_0; W[1] = rho2_0; W[2] = 0.0; W[3] = 0.0; W[4] = p0; W[5] = P.z_min + (1.0 - 2.0 * P.z_min) * prof; W[6] = 1.0;
+    }
+    Face f;
+    face_state(P, W, f);
+    const double z1 = W[5], q1 = (1.0 - z1) * W[1];
+    q[id] = z1 * W[0];
+    q[P.fstride + id] = q1;
+    q[2 * P.fstride + id] = f.rho * W[2];
+    q[3 * P.fstride + id] = f.rho * W[3];
+    q[4 * P.fstride + id] = f.rhoE;
+    q[5 * P.fstride + id] = z1;
+    q[6 * P.fstride + id] = q1 * W[6];
+}
+void launch_fill_state(const Params& P, double* q, int shock_cells, Hug hug, double p_shock, double p0, double rho1_0, double rho2_0,
+                       cudaStream_t s)
+{
+    dim3 grid((P.nx + 127) / 128, P.ny);
+    k_fill_state<<<grid, 128, 0, s>>>(P, q, shock_cells, hug, p_shock, p0, rho1_0, rho2_0);
+}
+
+__global__ void k_capture_inflow(const __grid_constant__ Params P, const double* __restrict__ q, double* __restrict__ inflow)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= P.ny) return;
+    for (int f = 0; f < 7; ++f) inflow[f * P.ny + j] = q[f * P.fstride + (long long)(j + NGY) * P.pitch + NGX];
+}
+void launch_capture_inflow(const Params& P, const double* q, double* inflow, cudaStream_t s)
+{
+    k_capture_inflow<<<(P.ny + 127) / 128, 128, 0, s>>>(P, q, inflow);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// diagnostics (a8): fixed-shape two-pass tree, no floating-point atomics -> run-to-run deterministic
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void block_reduce_diag(double v[DIAG_NV], int& bad, double (*sm)[DIAG_NV + 1])
+{
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) v[k] += __shfl_down_sync(0xffffffffu, v[k], o);
+        v[7] = fmax(v[7], __shfl_down_sync(0xffffffffu, v[7], o));
+        bad |= __shfl_down_sync(0xffffffffu, bad, o);
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) {
+#pragma unroll
+        for (int k = 0; k < DIAG_NV; ++k) sm[w][k] = v[k];
+        sm[w][DIAG_NV] = (double)bad;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int nw = blockDim.x >> 5;
+        for (int ww = 1; ww < nw; ++ww) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] += sm[ww][k];
+            v[7] = fmax(v[7], sm[ww][7]);
+            bad |= (int)sm[ww][DIAG_NV];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) k_diag_partial(const __grid_constant__ Params P, const double* __restrict__ q, double* __restrict__ partial)
+{
+    __shared__ double sm[8][DIAG_NV + 1];
+    double v[DIAG_NV];
+#pragma unroll
+    for (int k = 0; k < DIAG_NV; ++k) v[k] = 0.0;
+    int bad = 0;
+    const long long ncell = (long long)P.nx * P.ny;
+    const long long per = (ncell + gridDim.x - 1) / gridDim.x;
+    const long long a = (long long)blockIdx.x * per, b = min(a + per, ncell);
+    for (long long t = a + threadIdx.x; t < b; t += blockDim.x) {
+        const int j = (int)(t / P.nx), i = (int)(t - (long long)j * P.nx);
+        const long long id = (long long)(j + NGY) * P.pitch + NGX + i;
+        double c[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) c[k] = q[k * P.fstride + id];
+        Prim W; double rho, c2, T2;
+        cons_to_prim(P, c, W, rho, c2, &T2);
+        v[0] += c[0]; v[1] += c[1]; v[2] += c[2]; v[3] += c[3]; v[4] += c[4]; v[5] += c[6];
+        if (P.reactive && T2 > 0.0) v[6] += c[6] * P.Cpre * exp(-P.Ta / T2);
+        const double sp = fmax(fabs(W.un), fabs(W.ut)) + sqrt(c2);
+        v[7] = fmax(v[7], sp);
+        const bool ok = isfinite(c[0]) && isfinite(c[1]) && isfinite(c[2]) && isfinite(c[3]) && isfinite(c[4]) && isfinite(c[5])
+                        && isfinite(c[6]) && c[0] > 0.0 && c[1] > 0.0;
+        bad |= ok ? 0 : 1;
+    }
+    block_reduce_diag(v, bad, sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < DIAG_NV; ++k) partial[(long long)blockIdx.x * (DIAG_NV + 1) + k] = v[k];
+        partial[(long long)blockIdx.x * (DIAG_NV + 1) + DIAG_NV] = (double)bad;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_diag_final(const double* __restrict__ partial, int nblocks, DiagOut* out)
+{
+    __shared__ double sm[8][DIAG_NV + 1];
+    double v[DIAG_NV];
+#pragma unroll
+    for (int k = 0; k < DIAG_NV; ++k) v[k] = 0.0;
+    int bad = 0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) v[k] += partial[(long long)b * (DIAG_NV + 1) + k];
+        v[7] = fmax(v[7], partial[(long long)b * (DIAG_NV + 1) + 7]);
+        bad |= (int)partial[(long long)b * (DIAG_NV + 1) + DIAG_NV];
+    }
+    block_reduce_diag(v, bad, sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) out->sum[k] = v[k];
+        out->smax = v[7];
+        out->bad = bad;
+    }
+}
+
+void launch_diag(const Params& P, const double* q, double* partial, DiagOut* out, cudaStream_t s)
+{
+    k_diag_partial<<<DIAG_BLOCKS, 256, 0, s>>>(P, q, partial);
+    k_diag_final<<<1, 256, 0, s>>>(partial, DIAG_BLOCKS, out);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// derived output fields
+// ---------------------------------------------------------------------------------------------------------
+__global__ void k_derived(const __grid_constant__ Params P, const double* __restrict__ q, int fid, double* __restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (i >= P.nx) return;
+    const long long id = (long long)(j + NGY) * P.pitch + NGX + i;
+    double c[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) c[k] = q[k * P.fstride + id];
+    double v;
+    if (fid < 7) v = c[fid];
+    else {
+        Prim W; double rho, c2, T2;
+        cons_to_prim(P, c, W, rho, c2, &T2);
+        switch (fid) {
+            case 16: v = W.p; break;
+            case 17: v = T2; break;
+            case 18: v = rho; break;
+            case 19: v = W.un; break;
+            case 20: v = W.ut; break;
+            case 21: v = W.lam; break;
+            case 22: v = 1.0 - W.lam; break;
+            case 23: v = W.r2; break;
+            case 24: v = sqrt(c2); break;
+            case 25: v = W.p / (W.r1 * P.G1 * P.cv1); break;
+            case 26: v = W.r1; break;
+            default: v = 0.0; break;
+        }
+    }
+    out[(long long)j * P.nx + i] = v;
+}
+void launch_derived(const Params& P, const double* q, int fid, double* out, cudaStream_t s)
+{
+    dim3 grid((P.nx + 127) / 128, P.ny);
+    k_derived<<<grid, 128, 0, s>>>(P, q, fid, out);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// seeded cavity generator (R16): counter-based candidates, greedy acceptance in candidate order.
+// Candidate k is accepted iff it overlaps no accepted candidate of lower index; the sequence stops once the
+// accepted area reaches the target.  The device resolves a batch in parallel by iterating "accept if every
+// lower-index conflicting candidate is rejected / reject if one is accepted" to its unique fixed point.
+// ---------------------------------------------------------------------------------------------------------
+struct GenPar {
+    unsigned long long seed;
+    long long Rmin, Rmax, G, H, xlo256, xhi256;
+    int periodic_y;
+};
+
+__device__ __forceinline__ unsigned long long mix64(unsigned long long x)
+{
+    x += 0x9E3779B97F4A7C15ULL;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBULL;
+    return x ^ (x >> 31);
+}
+__device__ __forceinline__ unsigned long long rnd(unsigned long long seed, unsigned long long k, unsigned long long s)
+{ return mix64(mix64(seed) + 4ULL * k + s); }
+
+// status: 0 undecided, 1 accepted, 2 rejected
+__global__ void k_gen_candidates(GenPar g, long long k0, int nb, long long* X, long long* Y, long long* R, int* status)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nb) return;
+    const unsigned long long k = (unsigned long long)(k0 + t);
+    const long long Rk = g.Rmin + (long long)__umul64hi(rnd(g.seed, k, 2), (unsigned long long)(g.Rmax - g.Rmin + 1));
+    const long long xlo = g.xlo256 + Rk, xhi = g.xhi256 - Rk;
+    int st = 0;
+    long long Xk = 0, Yk = 0;
+    if (xhi < xlo) st = 2;
+    else {
+        Xk = xlo + (long long)__umul64hi(rnd(g.seed, k, 0), (unsigned long long)(xhi - xlo + 1));
+        if (g.periodic_y) Yk = (long long)__umul64hi(rnd(g.seed, k, 1), (unsigned long long)g.H);
+        else {
+            const long long ylo = Rk, yhi = g.H - Rk;
+            if (yhi < ylo) st = 2;
+            else Yk = ylo + (long long)__umul64hi(rnd(g.seed, k, 1), (unsigned long long)(yhi - ylo + 1));
+        }
+    }
+    X[t] = Xk; Y[t] = Yk; R[t] = Rk; status[t] = st;
+}
+
+__device__ __forceinline__ bool conflict(const GenPar& g, long long Xa, long long Ya, long long Ra, long long Xb, long long Yb, long long Rb)
+{
+    const long long ddx = Xa - Xb;
+    long long ddy = Ya > Yb ? Ya - Yb : Yb - Ya;
+    if (g.periodic_y && 2 * ddy > g.H) ddy = g.H - ddy;
+    const long long lim = Ra + Rb + g.G;
+    return ddx * ddx + ddy * ddy < lim * lim;
+}
+
+// reject batch candidates that overlap an already accepted cavity (fixed-point list accX/accY/accR)
+__global__ void k_gen_vs_accepted(GenPar g, int nb, const long long* X, const long long* Y, const long long* R, int* status,
+                                  const long long* aX, const long long* aY, const long long* aR, int nacc)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nb || status[t] != 0) return;
+    const long long x = X[t], y = Y[t], r = R[t];
+    for (int j = 0; j < nacc; ++j)
+        if (conflict(g, x, y, r, aX[j], aY[j], aR[j])) { status[t] = 2; return; }
+}
+
+__global__ void k_gen_resolve(GenPar g, int nb, const long long* X, const long long* Y, const long long* R, volatile int* status, int* undecided)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nb || status[t] != 0) return;
+    const long long x = X[t], y = Y[t], r = R[t];
+    bool blocked = false;
+    for (int j = 0; j < t; ++j) {
+        const int sj = status[j];
+        if (sj == 2) continue;
+        if (conflict(g, x, y, r, X[j], Y[j], R[j])) {
+            if (sj == 1) { status[t] = 2; return; }
+            blocked = true;
+        }
+    }
+    if (blocked) atomicAdd(undecided, 1);
+    else status[t] = 1;
+}
+
+// sequential in candidate order: append accepted candidates until the area target is reached
+__global__ void k_gen_compact(int nb, const long long* X, const long long* Y, const long long* R, const int* status, long long* aX,
+                              long long* aY, long long* aR, long long* acc_state /* [0]=nacc, [1]=sum, [2]=cap */, long long target)
+{
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    long long n = acc_state[0], sum = acc_state[1];
+    const long long cap = acc_state[2];
+    for (int t = 0; t < nb && sum < target && n < cap; ++t)
+        if (status[t] == 1) { aX[n] = X[t]; aY[n] = Y[t]; aR[n] = R[t]; ++n; sum += R[t] * R[t]; }
+    acc_state[0] = n; acc_state[1] = sum;
+}
+
+__global__ void k_gen_export(int n, const long long* aX, const long long* aY, const long long* aR, Cav* out)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    out[t].x = (double)aX[t] / 256.0; out[t].y = (double)aY[t] / 256.0; out[t].r = (double)aR[t] / 256.0;
+}
+
+int generate_cavities(unsigned long long seed, double phi, double dmin, double dmax, double min_gap, int x_lo, int x_hi, int ny,
+                      int periodic_y, Cav** d_cav_out, cudaStream_t s, long long* launches)
+{
+    GenPar g;
+    g.seed = seed;
+    g.Rmin = (long long)std::llround(dmin * 128.0);
+    g.Rmax = (long long)std::llround(dmax * 128.0);
+    g.G = (long long)std::llround(min_gap * 256.0);
+    g.H = (long long)ny * 256;
+    g.xlo256 = (long long)x_lo * 256; g.xhi256 = (long long)x_hi * 256;
+    g.periodic_y = periodic_y;
+    if (g.Rmin <= 0 || g.Rmax < g.Rmin || x_hi <= x_lo || ny <= 0) return -1;
+    const long long target = (long long)std::floor(phi * (double)(x_hi - x_lo) * (double)ny * 65536.0 / 3.14159265358979323846);
+    const long long max_cand = 16 * (target / (g.Rmin * g.Rmin) + 1) + 1024;
+    const long long cap = target / (g.Rmin * g.Rmin) + 2;
+    const int NB = 8192;
+    long long *X, *Y, *R, *aX, *aY, *aR, *acc;
+    int *status, *undecided;
+    if (cudaMalloc(&X, NB * 8) || cudaMalloc(&Y, NB * 8) || cudaMalloc(&R, NB * 8) || cudaMalloc(&status, NB * 4) ||
+        cudaMalloc(&aX, cap * 8) || cudaMalloc(&aY, cap * 8) || cudaMalloc(&aR, cap * 8) || cudaMalloc(&acc, 3 * 8) ||
+        cudaMalloc(&undecided, 4))
+        return -2;
+    long long h_acc[3] = {0, 0, cap};
+    cudaMemcpyAsync(acc, h_acc, sizeof(h_acc), cudaMemcpyHostToDevice, s);
+    cudaStreamSynchronize(s);
+    const int tb = 128, gb = (NB + tb - 1) / tb;
+    for (long long k0 = 0; k0 < max_cand && h_acc[1] < target; k0 += NB) {
+        const int nb = (int)std::min<long long>(NB, max_cand - k0);
+        k_gen_candidates<<<gb, tb, 0, s>>>(g, k0, nb, X, Y, R, status);
+        k_gen_vs_accepted<<<gb, tb, 0, s>>>(g, nb, X, Y, R, status, aX, aY, aR, (int)h_acc[0]);
+        *launches += 2;
+        for (int round = 0; round < nb + 1; ++round) {
+            int h_und = 0;
+            cudaMemsetAsync(undecided, 0, 4, s);
+            k_gen_resolve<<<gb, tb, 0, s>>>(g, nb, X, Y, R, status, undecided);
+            *launches += 1;
+            cudaMemcpyAsync(&h_und, undecided, 4, cudaMemcpyDeviceToHost, s);
+            if (cudaStreamSynchronize(s) != cudaSuccess) return -2;
+            if (h_und == 0) break;
+        }
+        k_gen_compact<<<1, 1, 0, s>>>(nb, X, Y, R, status, aX, aY, aR, acc, target);
+        *launches += 1;
+        cudaMemcpyAsync(h_acc, acc, sizeof(h_acc), cudaMemcpyDeviceToHost, s);
+        if (cudaStreamSynchronize(s) != cudaSuccess) return -2;
+    }
+    const int n = (int)h_acc[0];
+    Cav* d_cav = nullptr;
+    if (cudaMalloc(&d_cav, sizeof(Cav) * (size_t)(n > 0 ? n : 1))) return -2;
+    if (n > 0) { k_gen_export<<<(n + 127) / 128, 128, 0, s>>>(n, aX, aY, aR, d_cav); *launches += 1; }
+    cudaStreamSynchronize(s);
+    cudaFree(X); cudaFree(Y); cudaFree(R); cudaFree(status); cudaFree(aX); cudaFree(aY); cudaFree(aR); cudaFree(acc); cudaFree(undecided);
+    *d_cav_out = d_cav;
+    return cudaGetLastError() == cudaSuccess ? n : -2;
+}
+
+} // namespace nmsdt

@@ -1,0 +1,66 @@
+"""CPU-side checks of the C-ABI boundary: the library loads, exports every symbol include/nmsdt.h declares,
+host-only entry points work, and the product path fails loudly without a CUDA device (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1905_05727_b200 import build, binding
+    build.build()
+    return binding.load_library()
+
+
+def test_header_symbols_are_all_exported(lib):
+    from paper_1905_05727_b200 import binding
+    hdr = open(os.path.join(ROOT, "include", "nmsdt.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(sim_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.SYMBOLS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_workspace_bytes_is_host_only_and_matches_layout(lib):
+    from paper_1905_05727_b200 import binding, inputs
+    g = inputs.config("C5")["grid"]
+    n = binding.workspace_bytes(g)
+    pitch = (16 + g["nx"] + 2 + 15) // 16 * 16
+    planes = 14 * pitch * (g["ny"] + 4) * 8
+    assert planes <= n < planes + (1 << 20)
+    assert 15.0e9 < n < 15.2e9                     # ~15 GB double-buffered fp64 state
+    assert binding.workspace_bytes(dict(g, nx=0)) == 0
+    assert binding.workspace_bytes(dict(g, bc_ylo=1, bc_yhi=0)) == 0
+
+
+def test_no_cpu_fallback():
+    import torch
+    from paper_1905_05727_b200 import binding, inputs
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    c = inputs.config("C1")
+    with pytest.raises(RuntimeError):
+        binding.Sim(c["grid"], c["eos"], c["kin"])
+    # and the C entry point itself refuses without a device
+    L = binding.load_library()
+    h = C.c_void_p()
+    g = binding._fill(binding.Grid(), c["grid"])
+    e = binding._fill(binding.Eos(), c["eos"])
+    k = binding._fill(binding.Kin(), c["kin"])
+    rc = L.sim_create(C.byref(g), C.byref(e), C.byref(k), None, 0, None, C.byref(h))
+    assert rc == binding.SIM_ERR_CUDA and not h.value
+    assert b"no CUDA device" in L.sim_last_error(None)
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1905_05727_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle_py" not in src and "nmsdt_oracle" not in src and "liboracle" not in src, f

@@ -1,0 +1,318 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, same seeded inputs.
+
+Tolerances are BASELINE.json north_star's, all fp64: max relative difference in every conserved variable
+<= 1e-11 after one step (metric R18, tests/parity_util.py), L1-relative <= 1e-7 after 500 steps, global
+reaction-rate curve and overtake time within 0.5 %.  Integer work (cavity list) is bit-exact.
+Oracle inputs never come from the CUDA path: states are produced by the oracle and handed to the GPU.
+"""
+import numpy as np
+import pytest
+
+from paper_1905_05727_b200 import inputs
+from parity_util import TOL_L1_500, TOL_ONE_STEP, TOL_RATE, l1_rel, rel_diff
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1905_05727_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _pair(O, B, cfg, threads=8, variant=None):
+    o = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=threads)
+    s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=variant)
+    return o, s
+
+
+def _sync_state(o, s):
+    """hand the oracle's state to the GPU"""
+    s.init_fields(o.state())
+
+
+def _assert_one_step(o, s, tol=TOL_ONE_STEP, what=""):
+    qa, qb = s.state(), o.state()
+    r = rel_diff(qa, qb, o.read_field("c"))
+    assert max(r) <= tol, "%s rel diff per variable %s" % (what, r)
+    return r
+
+
+VARIANTS = [0, 1]
+
+
+# ------------------------------------------------------------------------------------------------ init
+def test_init_fields_round_trip_is_exact(O, B):
+    cfg = inputs.config("C1")
+    o, s = _pair(O, B, cfg)
+    o.init(cfg["init"])
+    _sync_state(o, s)
+    for a, b in zip(s.state(), o.state()):
+        assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("name,kw", [("C1", {}), ("C3", dict(nx=1024, ny=256)), ("C4", dict(nx=2048, ny=512)),
+                                     ("C5", dict(nx=2048, ny=512))])
+def test_sim_init_matches_oracle_init(O, B, name, kw):
+    cfg = inputs.config(name, **kw)
+    o, s = _pair(O, B, cfg)
+    o.init(cfg["init"])
+    s.init(cfg["init"])
+    ca, cb = s.cavities(), o.cavities()
+    assert ca.shape == cb.shape and np.array_equal(ca, cb)          # integer work: bit-exact
+    qa, qb = s.state(), o.state()
+    for k in range(7):
+        # q1, q6 carry z2 = 1 - z1: where z1 -> 1 - 1e-6 one ulp of tanh is 1e-10 of z2
+        np.testing.assert_allclose(qa[k], qb[k], rtol=1e-12, atol=1e-12 if k in (1, 6) else 0)
+    da, db = s.diagnostics(), o.diagnostics()
+    assert da["M2tot0"] == pytest.approx(db["M2tot0"], rel=1e-12)
+    assert s.cfl_dt() == pytest.approx(o.cfl_dt(), rel=1e-13)
+
+
+def test_generator_matches_oracle_at_full_c4_and_c5_sizes(O, B):
+    for name in ("C4", "C5"):
+        cfg = inputs.config(name)
+        ini, g = cfg["init"], cfg["grid"]
+        ref = O.gen_cavities(ini["seed"], ini["phi"], ini["dmin"], ini["dmax"], ini["min_gap"], ini["x_lo"], ini["x_hi"],
+                             g["ny"], 1)
+        # drive only the generator: a grid with the real ny but few columns would change x_hi, so use a thin
+        # dummy grid and the explicit generator parameters through sim_init on a narrow strip is not possible;
+        # C4 fits easily, C5's generator is checked on the full grid in test_full_size_sampled_parity.
+        if name == "C4":
+            s = B.Sim(g, cfg["eos"], cfg["kin"])
+            s.init(ini)
+            assert np.array_equal(s.cavities(), ref)
+            assert 400 < len(ref) < 600
+            s.close()
+        else:
+            assert 8000 < len(ref) < 13000
+
+
+# ------------------------------------------------------------------------------------------------ pieces
+def _developed_c1(O, reactive, steps=120, threads=8):
+    cfg = inputs.config("C1", reactive=reactive)
+    o = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=threads)
+    o.init(cfg["init"])
+    o.step(steps)
+    return cfg, o
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("d", [0, 1])
+def test_single_sweep_parity(O, B, d, variant):
+    cfg, o = _developed_c1(O, reactive=0, steps=400)       # shock inside the cavity: strong 2D structure
+    s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=variant)
+    _sync_state(o, s)
+    dt = o.cfl_dt()
+    o.sweep(d, dt)
+    s.sweep(d, dt)
+    _assert_one_step(o, s, what="sweep dir %d" % d)
+    assert o.fallback_count() == 0
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("bc", [0, 1, 2, 3])
+def test_halo_rules_through_sweeps(O, B, bc, variant):
+    # a small box whose activity touches every boundary; ragged sizes (not multiples of any tile)
+    nx, ny = 83, 37
+    bcx = (bc, bc if bc != 3 else 0)
+    bcy = (bc if bc != 3 else 1,) * 2
+    grid = dict(nx=nx, ny=ny, dx=4e-6, dy=4e-6, bc_xlo=bcx[0], bc_xhi=bcx[1], bc_ylo=bcy[0], bc_yhi=bcy[1], cfl=0.4, limiter=0)
+    kin = dict(inputs.KIN, reactive=0)
+    ini = dict(inputs._INIT0, p_shock=9e9, shock_cells=6, cavities=[(2.0, 3.0, 7.0), (80.0, 35.0, 6.0), (40.0, 0.0, 5.0)])
+    o = O.Oracle(grid, inputs.EOS, kin)
+    o.init(ini)
+    s = B.Sim(grid, inputs.EOS, kin, variant=variant)
+    _sync_state(o, s)
+    for it in range(6):                 # no re-sync: both sides keep their own state and step parity
+        dt = o.cfl_dt()
+        assert s.cfl_dt() == pytest.approx(dt, rel=1e-12)
+        o.step_dt(1, dt)
+        s.step_dt(1, dt)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="bc %d step %d" % (bc, it))
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_source_step_parity(O, B, variant):
+    cfg, o = _developed_c1(O, reactive=1, steps=400)
+    s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=variant)
+    _sync_state(o, s)
+    for tau in (1e-10, 5e-9):           # 5e-9: forces several RK4 sub-steps in the hot cells
+        o.source(tau)
+        s.source(tau)
+        r = _assert_one_step(o, s, what="source tau=%g" % tau)
+        _sync_state(o, s)
+    assert o.read_field("lambda")[:, 40:].min() < 0.999     # something burned outside the inert slab
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_diagnostics_and_cfl_parity(O, B, variant):
+    cfg, o = _developed_c1(O, reactive=1, steps=300)
+    s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=variant)
+    o2 = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"])
+    o2.init(cfg["init"])
+    s.init(cfg["init"])
+    m0 = s.diagnostics()["M2tot0"]
+    _sync_state(o, s)
+    assert s.cfl_dt() == pytest.approx(o.cfl_dt(), rel=1e-13)
+    da, db = s.diagnostics(), o.diagnostics()
+    for k in ("M2r", "mass1", "mass2", "momx", "energy", "rate_inst", "smax"):
+        assert da[k] == pytest.approx(db[k], rel=1e-12), k
+    assert abs(da["momy"] - db["momy"]) <= 1e-12 * abs(db["momx"])
+    assert da["bad_state"] == 0
+    # deterministic reduction: same bits twice
+    assert s.diagnostics() == da
+
+
+def test_derived_fields_parity(O, B):
+    cfg, o = _developed_c1(O, reactive=1, steps=200)
+    s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"])
+    _sync_state(o, s)
+    for name, tol in (("p", 1e-9), ("T2", 1e-9), ("rho", 1e-14), ("u", 1e-13), ("v", 1e-13), ("lambda", 1e-13),
+                      ("progress", 1e-13), ("rho2", 1e-13), ("c", 1e-10), ("rho1", 1e-13), ("T1", 1e-9)):
+        a, b = s.read_field(name), o.read_field(name)
+        scale = np.maximum(np.abs(b), np.max(np.abs(b)) * 1e-6 + 1e-300)
+        assert np.max(np.abs(a - b) / scale) < tol, name
+
+
+def test_bad_state_is_reported(O, B):
+    cfg = inputs.config("C1")
+    o, s = _pair(O, B, cfg)
+    o.init(cfg["init"])
+    q = o.state()
+    q[4][5, 7] = np.nan
+    s.init_fields(q)
+    with pytest.raises(B.NmsdtError) as e:
+        s.cfl_dt()
+    assert e.value.code == B.SIM_ERR_BAD
+    assert s.diagnostics(allow_bad=True)["bad_state"] == 1
+
+
+# ------------------------------------------------------------------------------------------------ whole steps
+ONE_STEP_CASES = [
+    ("C1", dict(reactive=0), 0), ("C1", dict(reactive=1), 0), ("C1", dict(reactive=1), 400),
+    ("C2", dict(nx=1024, ny=32, p_shock=11e9), 0), ("C2", dict(nx=1024, ny=8, p_shock=11e9), 1500),
+    ("C3", dict(nx=768, ny=192), 0), ("C4", dict(nx=1536, ny=384), 0), ("C5", dict(nx=1536, ny=384), 0),
+]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("name,kw,pre", ONE_STEP_CASES)
+def test_one_step_parity(O, B, name, kw, pre, variant):
+    cfg = inputs.config(name, **kw)
+    o, s = _pair(O, B, cfg, variant=variant)
+    o.init(cfg["init"])
+    t_pre = 0.0
+    if pre:
+        o.step(pre)
+        t_pre = o.diagnostics()["t"]
+        o2 = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=8)     # restart the step counter at 0 on both sides
+        o2.init_fields(o.state())
+        o, t_pre = o2, 0.0
+    _sync_state(o, s)
+    for it in range(2):                 # an even (X-Y) and an odd (Y-X) step; no re-sync in between
+        dt = o.cfl_dt()
+        o.step(1)
+        s.step(1)                       # the GPU takes its own device-side CFL dt
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="%s %s pre=%d step %d" % (name, kw, pre, it))
+        da, db = s.diagnostics(), o.diagnostics()
+        assert da["dt_last"] == pytest.approx(dt, rel=1e-12) and da["step"] == it + 1
+        assert da["t"] == pytest.approx(db["t"] - (0.0 if not pre else t_pre), rel=1e-12)
+    assert o.fallback_count() == 0
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_500_steps_l1_parity_c1(O, B, variant):
+    cfg = inputs.config("C1", reactive=1)
+    o, s = _pair(O, B, cfg, variant=variant)
+    o.init(cfg["init"])
+    s.init(cfg["init"])
+    o.step(500)
+    s.step(500)
+    da, db = s.diagnostics(), o.diagnostics()
+    assert da["step"] == db["step"] == 500
+    assert da["t"] == pytest.approx(db["t"], rel=1e-9)
+    l1 = l1_rel(s.state(), o.state())
+    assert max(l1) <= TOL_L1_500, l1
+    assert o.fallback_count() == 0
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_500_steps_l1_parity_random_cavities_crop(O, B, variant):
+    cfg = inputs.config("C4", nx=768, ny=192)
+    o, s = _pair(O, B, cfg, variant=variant)
+    o.init(cfg["init"])
+    s.init(cfg["init"])
+    assert len(o.cavities()) >= 5
+    o.step(500)
+    s.step(500)
+    l1 = l1_rel(s.state(), o.state())
+    assert max(l1) <= TOL_L1_500, l1
+
+
+def test_reaction_rate_curve_and_overtake_time(O, B):
+    # neat NM strip (C2 shape, cropped so the oracle finishes in seconds), 11 GPa: ignition within ~0.3 us
+    cfg = inputs.config("C2", nx=1024, ny=4, p_shock=11e9)
+    o, s = _pair(O, B, cfg, variant=1)
+    o.init(cfg["init"])
+    s.init(cfg["init"])
+    ta, Ma, tb, Mb = [0.0], [s.diagnostics()["M2r"]], [0.0], [o.diagnostics()["M2r"]]
+    for _ in range(220):                # sample every 10 steps (R14)
+        o.step(10)
+        s.step(10)
+        da, db = s.diagnostics(), o.diagnostics()
+        ta.append(da["t"]); Ma.append(da["M2r"]); tb.append(db["t"]); Mb.append(db["M2r"])
+    ta, Ma, tb, Mb = map(np.array, (ta, Ma, tb, Mb))
+    ra = np.abs(np.diff(Ma)) / np.diff(ta) / da["M2tot0"]
+    rb = np.abs(np.diff(Mb)) / np.diff(tb) / db["M2tot0"]
+    k = int(np.argmax(rb))
+    assert 20 < k < len(rb) - 5, "rate peak must lie inside the run (k=%d)" % k
+    sig = rb > 0.01 * rb[k]
+    assert np.max(np.abs(ra[sig] / rb[sig] - 1.0)) < TOL_RATE
+    t_a, t_b = 0.5 * (ta[1:] + ta[:-1])[int(np.argmax(ra))], 0.5 * (tb[1:] + tb[:-1])[k]
+    assert t_a == pytest.approx(t_b, rel=TOL_RATE)
+
+
+# ------------------------------------------------------------------------------------------------ full size
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+def test_full_size_sampled_parity(O, B, name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times: the GPU advances the whole grid,
+    the oracle recomputes sampled windows (window + 8-cell margin = 2 steps x 2 sweeps x radius 2)."""
+    cfg = inputs.config(name)
+    g = cfg["grid"]
+    s = B.Sim(g, cfg["eos"], cfg["kin"], variant=1)
+    s.init(cfg["init"])
+    cav = s.cavities()
+    if name != "C3":
+        ini = cfg["init"]
+        ref = O.gen_cavities(ini["seed"], ini["phi"], ini["dmin"], ini["dmax"], ini["min_gap"], ini["x_lo"], ini["x_hi"], g["ny"], 1)
+        assert np.array_equal(cav, ref)
+    d0 = s.diagnostics()
+    dt = 0.9 * s.cfl_dt()
+    nx, ny = g["nx"], g["ny"]
+    W, M = 48, 8
+    rng = np.random.default_rng(2024)
+    wins = [(96, 0), (nx - W - 2 * M, ny - W - 2 * M)]                 # shock front; far corner
+    for c in cav[rng.choice(len(cav), size=3, replace=False)]:          # around cavities
+        wins.append((int(np.clip(c[0] - W // 2 - M, 0, nx - W - 2 * M)), int(np.clip(c[1] - W // 2 - M, 0, ny - W - 2 * M))))
+    before = s.state()
+    s.step_dt(2, dt)
+    after = s.state()
+    d1 = s.diagnostics()
+    assert d1["step"] == 2 and d1["t"] == pytest.approx(2 * dt, rel=1e-14)
+    for (x0, y0) in wins:
+        sl = (slice(y0, y0 + W + 2 * M), slice(x0, x0 + W + 2 * M))
+        wg = dict(g, nx=W + 2 * M, ny=W + 2 * M, bc_xlo=0, bc_xhi=0, bc_ylo=0, bc_yhi=0)
+        o = O.Oracle(wg, cfg["eos"], cfg["kin"])
+        o.init_fields([a[sl] for a in before])
+        o.step_dt(2, dt)
+        qa = [a[sl][M:-M, M:-M] for a in after]
+        qb = [b[M:-M, M:-M] for b in o.state()]
+        r = rel_diff(qa, qb, o.read_field("c")[M:-M, M:-M])
+        assert max(r) <= 2 * TOL_ONE_STEP, "%s window %s: %s" % (name, (x0, y0), r)
+    # global invariants that hold at any size: phase masses change only through the x boundaries (inflow)
+    assert d1["mass2"] > d0["mass2"] and d1["bad_state"] == 0
+    assert abs(d1["momy"]) < 1e-9 * abs(d1["momx"]) or name != "C3"
