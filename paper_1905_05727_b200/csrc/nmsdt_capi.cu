@@ -1,6 +1,7 @@
 // nmsdt_capi.cu -- the C ABI of libnmsdt.so (include/nmsdt.h): handle, workspace layout, step orchestration.
 #include "../../include/nmsdt.h"
 #include "nmsdt_host.h"
+#include "nmsdt_math.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -19,7 +20,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct Layout {
     int pitch, rows;
     long long fstride;       // doubles
-    size_t off_A, off_B, off_inflow, off_partial, off_diag, off_ctl, off_scratch, total;
+    size_t off_A, off_B, off_inflow, off_partial, off_diag, off_ctl, off_scratch, off_tab, total;
 };
 
 Layout make_layout(int nx, int ny)
@@ -37,6 +38,7 @@ Layout make_layout(int nx, int ny)
     L.off_diag = o; o = align_up(o + sizeof(DiagOut), 256);
     L.off_ctl = o; o = align_up(o + sizeof(Ctl), 256);
     L.off_scratch = o; o = align_up(o + 8 * sizeof(double), 256);
+    L.off_tab = o; o = align_up(o + MATH_TAB_DOUBLES * sizeof(double), 256);
     L.total = o;
     return L;
 }
@@ -52,7 +54,7 @@ struct sim {
     cudaStream_t stream = nullptr;
     char* base = nullptr;
     bool owns = false;
-    double *A = nullptr, *B = nullptr, *inflow = nullptr, *partial = nullptr, *scratch = nullptr;
+    double *A = nullptr, *B = nullptr, *inflow = nullptr, *partial = nullptr, *scratch = nullptr, *tab = nullptr;
     DiagOut* d_diag = nullptr;
     Ctl* ctl = nullptr;
     Cav* d_cav = nullptr;
@@ -60,8 +62,10 @@ struct sim {
     bool inited = false;
     long long host_step = 0;        // mirrors ctl->step (step parity decides the sweep order)
     double M2tot0 = 0.0;
-    int variant = SIM_VARIANT_UNFUSED;
-    int use_graph = 0;
+    int variant = SIM_VARIANT_FUSED;
+    int use_graph = 1;
+    bool cfl_valid = false;         // fused path: ctl->dt / ctl->tsafe describe the current state and dt mode
+    double dt_mode = -1.0;          // dt_fixed the control block was last prepared for
     long long launches = 0;
     std::string err;
     // event profiling (sim_profile)
@@ -112,6 +116,7 @@ void fill_params(sim* s)
     P.A = e.A; P.B = e.B; P.C = e.C; P.D = e.D; P.rho02 = e.rho02; P.irho02 = 1.0 / e.rho02; P.cv2 = e.cv2; P.Tref2 = e.Tref2;
     P.kA = -e.A / (1.0 - e.C); P.kB = e.B / (1.0 - e.D); P.AC = e.A * e.C; P.BD = e.B * e.D;
     P.z_min = e.z_min; P.z_max = 1.0 - e.z_min;
+    P.C2 = e.C * LOG2E; P.D2 = e.D * LOG2E; P.iG2cv2 = 1.0 / (e.Gamma2 * e.cv2); P.tab = s->tab;
     P.Ta = k.Ta; P.Cpre = k.Cpre; P.Q = k.Q; P.theta0 = k.substep_theta; P.reactive = k.reactive; P.max_substeps = k.max_substeps;
 }
 
@@ -182,6 +187,30 @@ void enqueue_step_unfused(sim* s)
     s->host_step++;
 }
 
+// one full step on the fused path: [halo, S(dt/2)+sweep d1] [halo, sweep d2 + S(dt/2) + CFL partial] [ctl]
+void enqueue_step_fused(sim* s)
+{
+    cudaStream_t st = s->stream;
+    const Params& P = s->P;
+    const double* dtp = &s->ctl->dt;
+    const int d1 = (s->host_step & 1) ? 1 : 0, d2 = 1 - d1;
+    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->A, s->inflow, d1, st); }
+    { KTimer t(s, d1 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->A, s->B, dtp, s->ctl, d1, 1, st); }
+    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->B, s->inflow, d2, st); }
+    { KTimer t(s, d2 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->B, s->A, dtp, s->ctl, d2, 2, st); }
+    { KTimer t(s, SIM_K_CFL); launch_ctl(P, s->ctl, 1, st); }
+    s->launches += 5;
+    s->host_step++;
+}
+
+// fused path: make ctl->dt / ctl->tsafe valid for the current state (first step after init or after a piecewise call)
+void prepare_ctl_fused(sim* s)
+{
+    { KTimer t(s, SIM_K_CFL); launch_cfl(s->P, s->A, s->ctl, s->stream); }
+    launch_ctl(s->P, s->ctl, 0, s->stream);
+    s->launches += 2;
+}
+
 int finish_init(sim* s)
 {
     cudaStream_t st = s->stream;
@@ -191,6 +220,7 @@ int finish_init(sim* s)
     cudaStreamSynchronize(st);
     s->host_step = 0;
     s->inited = true;
+    s->cfl_valid = false;
     s->launches += 1;
     sim_diag_t d;
     s->M2tot0 = 0.0;
@@ -240,8 +270,14 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     s->inflow = (double*)(s->base + s->L.off_inflow); s->partial = (double*)(s->base + s->L.off_partial);
     s->d_diag = (DiagOut*)(s->base + s->L.off_diag); s->ctl = (Ctl*)(s->base + s->L.off_ctl);
     s->scratch = (double*)(s->base + s->L.off_scratch);
+    s->tab = (double*)(s->base + s->L.off_tab);
     fill_params(s);
     cudaMemsetAsync(s->base, 0, s->L.total, s->stream);
+    {
+        double htab[MATH_TAB_DOUBLES];
+        fill_math_tables(htab);
+        cudaMemcpyAsync(s->tab, htab, sizeof(htab), cudaMemcpyHostToDevice, s->stream);   // pageable source: staged before return
+    }
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) { int rc = check_cuda(nullptr, "sim_create"); sim_destroy(s); return rc ? rc : SIM_ERR_CUDA; }
     *out = s;
     return SIM_OK;
@@ -315,6 +351,7 @@ int sim_cfl_dt(sim_t* s, double* dt_out)
 {
     if (!s || !dt_out) return fail(s, SIM_ERR_ARG, "sim_cfl_dt: NULL argument");
     if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_cfl_dt: not initialised");
+    s->cfl_valid = false;
     launch_set_double(&s->ctl->dt_fixed, 0.0, s->stream);
     launch_cfl(s->P, s->A, s->ctl, s->stream);
     launch_finalize_dt(s->P, s->ctl, s->stream);
@@ -333,7 +370,15 @@ static int step_common(sim_t* s, int n, double dt_fixed)
     if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_step: not initialised");
     launch_set_double(&s->ctl->dt_fixed, dt_fixed, s->stream);
     s->launches++;
-    for (int it = 0; it < n; ++it) enqueue_step_unfused(s);
+    if (s->variant == SIM_VARIANT_UNFUSED) {
+        for (int it = 0; it < n; ++it) enqueue_step_unfused(s);
+        s->cfl_valid = false;
+        return check_cuda(s, "sim_step");
+    }
+    if (n == 0) return SIM_OK;
+    if (!s->cfl_valid || s->dt_mode != dt_fixed) prepare_ctl_fused(s);
+    for (int it = 0; it < n; ++it) enqueue_step_fused(s);
+    s->cfl_valid = true; s->dt_mode = dt_fixed;
     return check_cuda(s, "sim_step");
 }
 
@@ -358,10 +403,13 @@ int sim_sweep(sim_t* s, int dir, double dt)
 {
     if (!s || (dir != 0 && dir != 1) || !(dt > 0.0)) return fail(s, SIM_ERR_ARG, "sim_sweep: bad argument");
     if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_sweep: not initialised");
+    s->cfl_valid = false;
     launch_set_double(s->scratch, dt, s->stream);
+    launch_set_double(s->scratch + 1, 1e300, s->stream);
     launch_halo(s->P, s->A, s->inflow, dir, s->stream);
-    launch_sweep_march(s->P, s->A, s->B, s->scratch, dir, s->stream);
-    s->launches += 3;
+    if (s->variant == SIM_VARIANT_FUSED) launch_sweep_fused(s->P, s->A, s->B, s->scratch, s->ctl, dir, 0, s->stream);
+    else launch_sweep_march(s->P, s->A, s->B, s->scratch, dir, s->stream);
+    s->launches += 4;
     // keep the state in A: copy the interior planes back (parity-test helper, not on the hot path)
     cudaMemcpyAsync(s->A, s->B, (size_t)7 * s->P.fstride * sizeof(double), cudaMemcpyDeviceToDevice, s->stream);
     return check_cuda(s, "sim_sweep");
@@ -372,8 +420,13 @@ int sim_source(sim_t* s, double tau)
     if (!s || !(tau > 0.0)) return fail(s, SIM_ERR_ARG, "sim_source: bad argument");
     if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_source: not initialised");
     if (!s->P.reactive) return SIM_OK;
+    s->cfl_valid = false;
     launch_set_double(s->scratch, tau, s->stream);
-    launch_source(s->P, s->A, s->scratch, 1.0, s->stream);
+    if (s->variant == SIM_VARIANT_FUSED) {
+        launch_set_double(s->scratch + 1, host_tsafe(tau, s->k.Cpre, s->k.Ta, s->k.substep_theta), s->stream);
+        launch_source_fast(s->P, s->A, s->scratch, s->stream);
+        s->launches++;
+    } else launch_source(s->P, s->A, s->scratch, 1.0, s->stream);
     s->launches += 2;
     return check_cuda(s, "sim_source");
 }
@@ -431,7 +484,7 @@ int sim_get_cavities(sim_t* s, sim_cavity_t* host_out, int cap, int* n)
 int sim_set_variant(sim_t* s, int variant, int use_graph)
 {
     if (!s || (variant != SIM_VARIANT_UNFUSED && variant != SIM_VARIANT_FUSED)) return fail(s, SIM_ERR_ARG, "sim_set_variant: bad argument");
-    s->variant = variant; s->use_graph = use_graph ? 1 : 0;
+    s->variant = variant; s->use_graph = use_graph ? 1 : 0; s->cfl_valid = false;
     return SIM_OK;
 }
 

@@ -25,11 +25,15 @@ struct Params {
     // kinetics (Table III) + sub-step rule
     double Ta, Cpre, Q, theta0;
     int reactive, max_substeps;
+    // fused path (nmsdt_fused.cu): C log2(e), D log2(e), 1/(Gamma2 cv2), device copy of the nmsdt_math.cuh tables
+    double C2, D2, iG2cv2;
+    const double* tab;
 };
 
 // device-resident control block: the time step never visits the host inside sim_step
 struct Ctl {
     double dt;                    // step to take next
+    double tsafe;                 // T2 bound below which the R13 rule gives n_sub = 1 for tau = dt/2 (must follow dt)
     double t;
     double dt_last;
     double dt_fixed;              // > 0: sim_step_dt mode

@@ -1,0 +1,539 @@
+// nmsdt_fused.cu -- the production step kernels of libnmsdt.so (SIM_VARIANT_FUSED; fp64, sm_100a).
+//
+// One time step (O6; Strang splitting P:149) is two passes over the state:
+//   pass 1 = S(dt/2) applied on load + directional sweep d1          (k_xsweep<LEAD> or k_ysweep<LEAD>)
+//   pass 2 = directional sweep d2 + S(dt/2) on the updated cell + max-wavespeed partial of the new state
+//                                                                     (k_xsweep<TRAIL> or k_ysweep<TRAIL>)
+// followed by the one-thread k_ctl (t += dt, next CFL dt).  Algorithmic HBM traffic: 2 x (7 read + 7 written) planes
+// = 224 B per cell-step.  The arithmetic is that of nmsdt_device.cuh (O3-O5) with the branch-free elementary
+// functions of nmsdt_math.cuh.
+//
+//   k_ysweep: a thread owns a column and marches along y; the 3-cell primitive window, the previous right-face state
+//             and the half-finished update of the previous cell stay in registers; every load/store is a coalesced
+//             256-byte row piece and nothing is recomputed (4 ramp-up rows per segment).
+//   k_xsweep: a warp owns a row segment and marches along x in chunks of 64 cells, 2 adjacent cells per lane
+//             (128-bit loads/stores).  Neighbour primitives, the right-face state and the face flux cross lanes through
+//             three 33-slot rings in shared memory (slot = lane counter mod 33, so lane 31's entry of the previous
+//             chunk is lane 0's left neighbour: no halo recomputation, no copies); 3 __syncwarp per chunk.
+#include "nmsdt_host.h"
+#include "nmsdt_math.cuh"
+
+namespace nmsdt {
+
+namespace {
+
+enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2 };
+
+struct FCell {            // W = (rho1, rho2, un, ut, p, z1, lambda) + what the Hancock predictor needs
+    double r1, r2, un, ut, p, z1, lam;
+    double irho, rc2;     // 1/rho, rho c^2 (with the c >= 1 m/s floor of R10)
+};
+struct FFace { double r1, r2, un, ut, p, z1, lam, rho, rhoE, c; };
+
+__device__ __forceinline__ double clampf(double x, double lo, double hi) { return fmin(fmax(x, lo), hi); }
+
+// R13 exact sub-step count (only reached by cells hotter than the safe bound; same exactly-rounded sequence as k_source)
+__device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
+{
+    if (!(Tub > 0.0)) return 1;
+    double y = __ddiv_rn(P.Ta, Tub);
+    double y2 = __dmul_rn(y, y);
+    double den = __dadd_rn(__dadd_rn(__dadd_rn(1.0, y), __ddiv_rn(y2, 2.0)), __ddiv_rn(__dmul_rn(y2, y), 6.0));
+    double g = __ddiv_rn(1.0, den);
+    double theta = __dmul_rn(__dmul_rn(tau, P.Cpre), g);
+    double r = floor(__ddiv_rn(theta, P.theta0));
+    return (r >= (double)(P.max_substeps - 1)) ? P.max_substeps : 1 + (int)r;
+}
+
+// O5: lambda after integrating d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)) over tau, T2 = T0 + beta (lam0 - lambda)
+__device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0,
+                                                double tau, double Tsafe)
+{
+    const double Tub = fma(beta, lam0, T0);
+    int nsub = 1;
+    double h = tau;
+    if (Tub >= Tsafe) { nsub = nsub_exact(P, Tub, tau); h = tau / (double)nsub; }
+    const double nTa = P.Ta, mC = -P.Cpre;
+    double lam = lam0;
+    for (int s = 0; s < nsub; ++s) {
+        double l, T, k1, k2, k3, k4;
+        l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = T > 0.0 ? k1 : 0.0;
+        l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = T > 0.0 ? k2 : 0.0;
+        l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = T > 0.0 ? k3 : 0.0;
+        l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = T > 0.0 ? k4 : 0.0;
+        lam = fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
+    }
+    return clampf(lam, 0.0, lam0);
+}
+
+// O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.
+// SRC: the Arrhenius step over tau is applied to the cell; dE = energy moved into rho E, q6n = new z2 rho2 lambda.
+template <bool SRC>
+__device__ __forceinline__ void prim_cell(const Params& P, const double* __restrict__ tab, const double q[7], double tau, double Tsafe,
+                                          FCell& W, double& dE, double& q6n)
+{
+    const double rho = q[0] + q[1];
+    const double irho = q_rcp(rho);
+    W.irho = irho;
+    W.un = q[2] * irho;
+    W.ut = q[3] * irho;
+    const double z1 = clampf(q[5], P.z_min, P.z_max);
+    const double z2 = 1.0 - z1;
+    const double iq1 = q_rcp(q[1]);
+    W.z1 = z1;
+    W.r1 = q[0] * q_rcp(z1);
+    W.r2 = q[1] * q_rcp(z2);
+    const double rhoe = fma(-0.5 * irho, fma(q[2], q[2], q[3] * q[3]), q[4]);
+    const double x = W.r2 * P.irho02;
+    double xC, xD;
+    q_pow_pair(tab, x, P.C2, P.D2, xC, xD);
+    const double pr = fma(P.A, xC, -P.B * xD);                                   // Eq. 3
+    const double rer = fma(P.kA, xC - x, P.kB * (xD - x));                       // rho2 * Eq. 4
+    const double xi = fma(z1, P.iG1, z2 * P.iG2);
+    const double ixi = q_rcp(xi);
+    double p = (rhoe - z2 * fma(-pr, P.iG2, rer)) * ixi;
+    double lam = clampf(q[6] * iq1, 0.0, 1.0);
+    dE = 0.0; q6n = q[6];
+    if (SRC) {
+        if (P.reactive) {
+            const double T0 = P.Tref2 + (p - pr) * (z2 * iq1) * P.iG2cv2;        // Eq. 5 (1/rho2 = z2/q1)
+            const double beta = z2 * P.Q * ixi * P.iG2cv2;
+            const double lam1 = arrhenius_rk4(P, tab, T0, beta, lam, tau, Tsafe);
+            dE = q[1] * P.Q * (lam - lam1);
+            q6n = q[1] * lam1;
+            p = fma(dE, ixi, p);                                                 // p is linear in rho e at frozen rho_k, z_k
+            lam = lam1;
+        }
+    }
+    W.p = p; W.lam = lam;
+    const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
+    const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22) * ixi;  // R10
+    W.rc2 = fmax(rc2, rho);                                                      // c^2 >= 1
+}
+
+__device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f)
+{
+    const double z1 = W[5], z2 = 1.0 - z1, p = W[4];
+    f.r1 = W[0]; f.r2 = W[1]; f.un = W[2]; f.ut = W[3]; f.p = p; f.z1 = z1; f.lam = W[6];
+    const double rho = fma(z1, W[0], z2 * W[1]);
+    f.rho = rho;
+    const double x = W[1] * P.irho02;
+    double xC, xD;
+    q_pow_pair(tab, x, P.C2, P.D2, xC, xD);
+    const double pr = fma(P.A, xC, -P.B * xD);
+    const double rer = fma(P.kA, xC - x, P.kB * (xD - x));
+    const double kin = 0.5 * rho * fma(W[2], W[2], W[3] * W[3]);
+    f.rhoE = fma(z1 * P.iG1, p, fma(z2, fma(p - pr, P.iG2, rer), kin));
+    const double xi = fma(z1, P.iG1, z2 * P.iG2);
+    const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
+    const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22);
+    f.c = q_sqrt(fmax(rc2 * q_rcp(xi * rho), 1.0));
+}
+
+__device__ __forceinline__ double limited_f(int kind, double a, double b)
+{
+    const double ab = a * b;
+    double m;
+    if (kind == 0) m = fabs(a) < fabs(b) ? a : b;                                 // minmod (R5)
+    else { m = fmin(fmin(2.0 * fabs(a), 2.0 * fabs(b)), 0.5 * fabs(a + b)); m = a > 0.0 ? m : -m; }
+    return ab > 0.0 ? m : 0.0;
+}
+
+// O4.1-2 for the centre cell W0
+__device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, const FCell& W0, const FCell& Wp, double khalf, double WL[7],
+                                           double WR[7])
+{
+    const double w0[7] = {W0.r1, W0.r2, W0.un, W0.ut, W0.p, W0.z1, W0.lam};
+    const double wm[7] = {Wm.r1, Wm.r2, Wm.un, Wm.ut, Wm.p, Wm.z1, Wm.lam};
+    const double wp[7] = {Wp.r1, Wp.r2, Wp.un, Wp.ut, Wp.p, Wp.z1, Wp.lam};
+    double D[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) D[k] = limited_f(P.limiter, w0[k] - wm[k], wp[k] - w0[k]);
+    const double u = W0.un;
+    double d[7];
+    d[0] = fma(u, D[0], W0.r1 * D[2]);
+    d[1] = fma(u, D[1], W0.r2 * D[2]);
+    d[2] = fma(u, D[2], D[4] * W0.irho);
+    d[3] = u * D[3];
+    d[4] = fma(u, D[4], W0.rc2 * D[2]);
+    d[5] = u * D[5];
+    d[6] = u * D[6];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        const double m = fma(-khalf, d[k], w0[k]);
+        WL[k] = fma(-0.5, D[k], m);
+        WR[k] = fma(0.5, D[k], m);
+    }
+    const bool ok = (WL[0] > 0.0) && (WL[1] > 0.0) && (WR[0] > 0.0) && (WR[1] > 0.0);     // R17
+    if (!ok) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) { WL[k] = w0[k]; WR[k] = w0[k]; }
+    }
+}
+
+// O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
+__device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double F[8])
+{
+    const double SL = fmin(L.un - L.c, R.un - R.c);                  // R9: Davis
+    const double SR = fmax(L.un + L.c, R.un + R.c);
+    const double mL = L.rho * (SL - L.un), mR = R.rho * (SR - R.un);
+    const double Sstar = (R.p - L.p + fma(L.un, mL, -R.un * mR)) * q_rcp(mL - mR);
+    const bool useL = (SL >= 0.0) || ((SR > 0.0) && (Sstar >= 0.0));
+    const bool star = (SL < 0.0) && (SR > 0.0);
+    const double r1 = useL ? L.r1 : R.r1, r2 = useL ? L.r2 : R.r2, un = useL ? L.un : R.un, ut = useL ? L.ut : R.ut;
+    const double p = useL ? L.p : R.p, z1 = useL ? L.z1 : R.z1, lam = useL ? L.lam : R.lam;
+    const double rho = useL ? L.rho : R.rho, rhoE = useL ? L.rhoE : R.rhoE, SK = useL ? SL : SR;
+    double U[7], FK[7];
+    U[0] = z1 * r1; U[1] = (1.0 - z1) * r2; U[2] = rho * un; U[3] = rho * ut; U[4] = rhoE; U[5] = z1; U[6] = U[1] * lam;
+    FK[0] = U[0] * un; FK[1] = U[1] * un; FK[2] = fma(U[2], un, p); FK[3] = U[2] * ut; FK[4] = (rhoE + p) * un;
+    FK[5] = z1 * un; FK[6] = U[6] * un;
+    // chi = (SK-un)/(SK-S*), p/(SK-un) from one reciprocal
+    const double a = SK - un, b = SK - Sstar;
+    const double rab = star ? q_rcp(a * b) : 0.0;                     // keeps the unused star state finite outside the fan
+    const double chi = a * a * rab;
+    const double poa = p * b * rab;
+    double Us[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) Us[k] = chi * U[k];
+    Us[2] = rho * chi * Sstar;
+    Us[4] = chi * fma(Sstar - un, fma(rho, Sstar, poa), rhoE);
+    const double SKs = star ? SK : 0.0;                               // F = FK + SK (U* - U) in the star region, FK otherwise
+#pragma unroll
+    for (int k = 0; k < 7; ++k) F[k] = fma(SKs, Us[k] - U[k], FK[k]);
+    F[7] = fma(SKs, chi - 1.0, un);
+}
+
+__device__ __forceinline__ bool all_finite7(const double o[7])
+{
+    int m = 0;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) m = max(m, __double2hiint(o[k]) & 0x7fffffff);
+    return m < 0x7ff00000;
+}
+
+// finished cell of the second pass: trailing S(dt/2), wavespeed of the new state, state check (a6, a7, R17)
+__device__ __forceinline__ void trail_cell(const Params& P, const double* __restrict__ tab, double o[7], double tau, double Tsafe, double& smax,
+                                           int& bad)
+{
+    FCell W; double dE, q6n;
+    prim_cell<true>(P, tab, o, tau, Tsafe, W, dE, q6n);
+    o[4] += dE; o[6] = q6n;
+    const double a = fmax(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
+    const bool ok = all_finite7(o) && o[0] > 0.0 && o[1] > 0.0 && (__double2hiint(a) & 0x7fffffff) < 0x7ff00000;
+    bad |= ok ? 0 : 1;
+    smax = fmax(smax, a);
+}
+
+__device__ __forceinline__ void reduce_smax(double smax, int bad, Ctl* ctl)
+{
+    for (int o = 16; o > 0; o >>= 1) {
+        smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+        bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(&ctl->smax_bits, dbits(smax));
+        if (bad) atomicOr(&ctl->bad, 1);
+    }
+}
+
+// post-source conserved values of a cell whose post-source lambda is known (pass 1 applies S on load, O6)
+__device__ __forceinline__ void lead_fix(const Params& P, double q[7], double lam1)
+{
+    if (P.reactive) {
+        const double q6n = q[1] * lam1;
+        q[4] = fma(P.Q, q[6] - q6n, q[4]);
+        q[6] = q6n;
+    }
+}
+
+constexpr int XW = 4;                       // warps per block in k_xsweep
+constexpr int RING = 33;
+constexpr int RING_DOUBLES = (16 + 10 + 8) * RING;
+
+} // namespace
+
+// ---------------------------------------------------------------------------------------------------------------
+// y-sweep (a5): thread per column, register marching
+// ---------------------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(128) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
+                                                const double* __restrict__ dtp, Ctl* ctl, int seg)
+{
+    __shared__ double s_tab[MATH_TAB_DOUBLES];
+    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
+    __syncthreads();
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    double smax = 0.0; int bad = 0;
+    if (col < P.nx) {
+        const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
+        const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
+        const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
+        const long long fs = P.fstride, pitch = P.pitch;
+        const double* pin = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
+        double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
+        FCell Wm, W0, Wp;
+        Wm = W0 = FCell{1, 1, 0, 0, 1, 0.5, 0, 1, 1};
+        FFace prevR = FFace{1, 1, 0, 0, 1, 0.5, 0, 1, 1, 1};
+        double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
+        for (int c = c0 - 2; c < c1 + 2; ++c, pin += pitch) {
+            double q[7];
+            q[0] = pin[0]; q[1] = pin[fs]; q[2] = pin[3 * fs]; q[3] = pin[2 * fs]; q[4] = pin[4 * fs]; q[5] = pin[5 * fs]; q[6] = pin[6 * fs];
+            double dE, q6n;
+            prim_cell<MODE == MODE_LEAD>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n);
+            const int jj = c - (c0 - 2);
+            if (jj >= 2) {                       // centre cell c-1 has both neighbours
+                double WL[7], WR[7];
+                recon_fast(P, Wm, W0, Wp, khalf, WL, WR);
+                if (jj >= 3) {
+                    FFace fl;
+                    face_fast(P, s_tab, WL, fl);
+                    double F[8];
+                    hllc_fast(prevR, fl, F);     // face between cells c-2 and c-1
+                    if (jj >= 4) {               // finish cell c-2
+                        double o[7];
+#pragma unroll
+                        for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
+                        o[5] = fma(dtdx * z1n, F[7], o[5]);                       // R8: non-conservative z1 term
+                        o[5] = clampf(o[5], P.z_min, P.z_max);
+                        if (MODE == MODE_TRAIL) trail_cell(P, s_tab, o, tau, Tsafe, smax, bad);
+                        pout[0] = o[0]; pout[fs] = o[1]; pout[3 * fs] = o[2]; pout[2 * fs] = o[3]; pout[4 * fs] = o[4]; pout[5 * fs] = o[5];
+                        pout[6 * fs] = o[6];
+                        pout += pitch;
+                    }
+                    if (c - 1 < c1) {            // start cell c-1 with its lower-face flux
+                        const double* pc = pin - pitch;
+                        double o[7];
+                        o[0] = pc[0]; o[1] = pc[fs]; o[2] = pc[3 * fs]; o[3] = pc[2 * fs]; o[4] = pc[4 * fs]; o[5] = pc[5 * fs]; o[6] = pc[6 * fs];
+                        if (MODE == MODE_LEAD) lead_fix(P, o, W0.lam);
+                        z1n = o[5];
+#pragma unroll
+                        for (int k = 0; k < 7; ++k) acc[k] = fma(dtdx, F[k], o[k]);
+                        acc[5] = fma(-dtdx * z1n, F[7], acc[5]);
+                    }
+                }
+                face_fast(P, s_tab, WR, prevR);
+            }
+            Wm = W0; W0 = Wp;
+        }
+    }
+    if (MODE == MODE_TRAIL) reduce_smax(smax, bad, ctl);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// x-sweep (a4): warp per row segment, 2 cells per lane, shared-memory rings between lanes
+// ---------------------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
+                                                    const double* __restrict__ dtp, Ctl* ctl, int seg)
+{
+    __shared__ double s_tab[MATH_TAB_DOUBLES];
+    __shared__ double s_ring[XW * RING_DOUBLES];
+    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int row = blockIdx.x * XW + warp;
+    double smax = 0.0; int bad = 0;
+    if (row < P.ny) {
+        double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
+        double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
+        double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
+        const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
+        const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
+        const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
+        const long long fs = P.fstride;
+        const double* rin = qin + (long long)(row + NGY) * P.pitch + NGX;
+        double* rout = qout + (long long)(row + NGY) * P.pitch + NGX;
+        const int nxe = (P.nx + 1) & ~1;                 // last pair base that is ever needed (cell nx+1 is the outer ghost; for odd nx the pair ends in row padding)
+        const int niter = (c1 - c0 + 63) >> 6;
+        const bool fixed_in = (MODE == MODE_LEAD) && (P.bc_xlo == 3);
+        int sw = lane;                                   // ring slot written by this lane: (32 k + lane) mod 33
+        for (int k = 0; k <= niter; ++k) {
+            const int b = c0 + 64 * (k - 1);             // first cell updated in this iteration
+            const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
+            const bool act = (k > 0) || (lane >= 30);    // iteration 0 only primes the rings (cells c0-2 .. c0+1)
+            const int sr = sw == 0 ? RING - 1 : sw - 1;  // left neighbour's slot
+            FCell WA, WB;
+            // ---- phase 1: load, primitives (+ leading source) ----------------------------------------------------
+            if (act) {
+                const int Ac = min(A, nxe);
+                const double* pa = rin + Ac;
+                double qa[7], qb[7];
+#pragma unroll
+                for (int f = 0; f < 7; ++f) { const double2 v = *reinterpret_cast<const double2*>(pa + f * fs); qa[f] = v.x; qb[f] = v.y; }
+                double dE, q6n;
+                prim_cell<MODE == MODE_LEAD>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n);
+                prim_cell<MODE == MODE_LEAD>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n);
+                rw[0 * RING + sw] = WA.r1; rw[1 * RING + sw] = WA.r2; rw[2 * RING + sw] = WA.un; rw[3 * RING + sw] = WA.ut;
+                rw[4 * RING + sw] = WA.p;  rw[5 * RING + sw] = WA.z1; rw[6 * RING + sw] = WA.lam;
+                rw[7 * RING + sw] = WB.r1; rw[8 * RING + sw] = WB.r2; rw[9 * RING + sw] = WB.un; rw[10 * RING + sw] = WB.ut;
+                rw[11 * RING + sw] = WB.p; rw[12 * RING + sw] = WB.z1; rw[13 * RING + sw] = WB.lam;
+                rw[14 * RING + sw] = WB.irho; rw[15 * RING + sw] = WB.rc2;
+            }
+            __syncwarp();
+            // ---- phase 2: reconstruct cells A-1 and A, four face states ------------------------------------------
+            FFace FL1, FR1, FL2;
+            double lam_u0 = 0.0, lam_u1 = 0.0;
+            if (act) {
+                FCell Wmm, Wm1;
+                Wmm.r1 = rw[0 * RING + sr]; Wmm.r2 = rw[1 * RING + sr]; Wmm.un = rw[2 * RING + sr]; Wmm.ut = rw[3 * RING + sr];
+                Wmm.p = rw[4 * RING + sr];  Wmm.z1 = rw[5 * RING + sr]; Wmm.lam = rw[6 * RING + sr]; Wmm.irho = 0.0; Wmm.rc2 = 0.0;
+                Wm1.r1 = rw[7 * RING + sr]; Wm1.r2 = rw[8 * RING + sr]; Wm1.un = rw[9 * RING + sr]; Wm1.ut = rw[10 * RING + sr];
+                Wm1.p = rw[11 * RING + sr]; Wm1.z1 = rw[12 * RING + sr]; Wm1.lam = rw[13 * RING + sr];
+                Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
+                lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
+                double WL[7], WR[7];
+                recon_fast(P, Wmm, Wm1, WA, khalf, WL, WR);
+                face_fast(P, s_tab, WL, FL1);
+                face_fast(P, s_tab, WR, FR1);
+                recon_fast(P, Wm1, WA, WB, khalf, WL, WR);
+                face_fast(P, s_tab, WL, FL2);
+                FFace FR2;
+                face_fast(P, s_tab, WR, FR2);
+                rfr[0 * RING + sw] = FR2.r1; rfr[1 * RING + sw] = FR2.r2; rfr[2 * RING + sw] = FR2.un; rfr[3 * RING + sw] = FR2.ut;
+                rfr[4 * RING + sw] = FR2.p;  rfr[5 * RING + sw] = FR2.z1; rfr[6 * RING + sw] = FR2.lam; rfr[7 * RING + sw] = FR2.rho;
+                rfr[8 * RING + sw] = FR2.rhoE; rfr[9 * RING + sw] = FR2.c;
+            }
+            __syncwarp();
+            // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
+            double F1[8], F2[8];
+            if (act) {
+                FFace FRp;
+                FRp.r1 = rfr[0 * RING + sr]; FRp.r2 = rfr[1 * RING + sr]; FRp.un = rfr[2 * RING + sr]; FRp.ut = rfr[3 * RING + sr];
+                FRp.p = rfr[4 * RING + sr];  FRp.z1 = rfr[5 * RING + sr]; FRp.lam = rfr[6 * RING + sr]; FRp.rho = rfr[7 * RING + sr];
+                FRp.rhoE = rfr[8 * RING + sr]; FRp.c = rfr[9 * RING + sr];
+                hllc_fast(FRp, FL1, F1);
+                hllc_fast(FR1, FL2, F2);
+#pragma unroll
+                for (int f = 0; f < 8; ++f) rf[f * RING + sw] = F2[f];
+            }
+            __syncwarp();
+            // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
+            const int u0 = b + 2 * lane;
+            if (k > 0 && u0 < c1) {
+                double F0[8];
+#pragma unroll
+                for (int f = 0; f < 8; ++f) F0[f] = rf[f * RING + sr];
+                const double* pu = rin + u0;
+                double oa[7], ob[7];
+#pragma unroll
+                for (int f = 0; f < 7; ++f) { const double2 v = *reinterpret_cast<const double2*>(pu + f * fs); oa[f] = v.x; ob[f] = v.y; }
+                if (MODE == MODE_LEAD) {
+                    lead_fix(P, oa, lam_u0);
+                    lead_fix(P, ob, lam_u1);
+                }
+                const double za = oa[5], zb = ob[5];
+#pragma unroll
+                for (int f = 0; f < 7; ++f) { oa[f] = fma(-dtdx, F1[f] - F0[f], oa[f]); ob[f] = fma(-dtdx, F2[f] - F1[f], ob[f]); }
+                oa[5] = clampf(fma(dtdx * za, F1[7] - F0[7], oa[5]), P.z_min, P.z_max);       // R8
+                ob[5] = clampf(fma(dtdx * zb, F2[7] - F1[7], ob[5]), P.z_min, P.z_max);
+                const bool two = u0 + 1 < c1;
+                if (MODE == MODE_TRAIL) {
+                    trail_cell(P, s_tab, oa, tau, Tsafe, smax, bad);
+                    double sm2 = 0.0; int bad2 = 0;
+                    trail_cell(P, s_tab, ob, tau, Tsafe, sm2, bad2);
+                    if (two) { smax = fmax(smax, sm2); bad |= bad2; }
+                }
+                double* po = rout + u0;
+                if (two) {
+#pragma unroll
+                    for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
+                } else {
+#pragma unroll
+                    for (int f = 0; f < 7; ++f) po[f * fs] = oa[f];
+                }
+            }
+            sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
+        }
+    }
+    if (MODE == MODE_TRAIL) reduce_smax(smax, bad, ctl);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pointwise source step with the fused-path arithmetic (sim_source under SIM_VARIANT_FUSED), in place
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_source_fast(const __grid_constant__ Params P, double* __restrict__ q, const double* __restrict__ dtp)
+{
+    __shared__ double s_tab[MATH_TAB_DOUBLES];
+    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (i >= P.nx) return;
+    const long long id = (long long)(j + NGY) * P.pitch + NGX + i;
+    double c[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) c[k] = q[k * P.fstride + id];
+    FCell W; double dE, q6n;
+    prim_cell<true>(P, s_tab, c, dtp[0], dtp[1], W, dE, q6n);
+    q[4 * P.fstride + id] = c[4] + dE;
+    q[6 * P.fstride + id] = q6n;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// one-thread control kernel: finish the step (t, step counter), next dt from the max wavespeed (a7, R11) and the
+// temperature bound below which the R13 rule certainly gives n_sub = 1 for tau = dt/2
+// ---------------------------------------------------------------------------------------------------------------
+__host__ __device__ inline double tsafe_for(double tau, double Cpre, double Ta, double theta0)
+{
+    // n_sub = 1 + floor(tau C g(Ta/T) / theta0), g(y) = 1/(1 + y + y^2/2 + y^3/6) decreasing in y.
+    // Return T* such that T < T* guarantees tau C g < theta0 (1 - 1e-6); +inf when that holds for every T.
+    const double target = theta0 * (1.0 - 1e-6) / (tau * Cpre);       // need g(y) < target
+    if (!(tau > 0.0) || target >= 1.0) return 1e300;
+    double lo = 0.0, hi = 1.0;                                        // g(lo) >= target > g(hi)
+    while (1.0 / (1.0 + hi * (1.0 + hi * (0.5 + hi / 6.0))) >= target) hi *= 2.0;
+    for (int it = 0; it < 64; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (1.0 / (1.0 + mid * (1.0 + mid * (0.5 + mid / 6.0))) >= target) lo = mid; else hi = mid;
+    }
+    return Ta / hi;                                                   // T < Ta/hi  =>  y > hi  =>  g(y) < target
+}
+
+__global__ void k_ctl(const __grid_constant__ Params P, Ctl* ctl, int advance)
+{
+    if (advance) { ctl->t += ctl->dt; ctl->dt_last = ctl->dt; ctl->step += 1; }
+    const double smax = __longlong_as_double((long long)ctl->smax_bits);
+    const double dt = ctl->dt_fixed > 0.0 ? ctl->dt_fixed : P.cfl * P.hmin / smax;
+    ctl->dt = dt;
+    ctl->tsafe = P.reactive ? tsafe_for(0.5 * dt, P.Cpre, P.Ta, P.theta0) : 1e300;
+    ctl->smax_bits = 0ull;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------------------------
+static int pick_seg(int n, int unit, int target)
+{
+    int nseg = (n + target - 1) / target;
+    if (nseg < 1) nseg = 1;
+    int seg = (n + nseg - 1) / nseg;
+    return (seg + unit - 1) / unit * unit;
+}
+
+void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s)
+{
+    if (dir == 0) {
+        const int seg = pick_seg(P.nx, 64, 2048);
+        dim3 grid((P.ny + XW - 1) / XW, (P.nx + seg - 1) / seg);
+        if (mode == MODE_PLAIN)      k_xsweep<MODE_PLAIN><<<grid, 32 * XW, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_LEAD)  k_xsweep<MODE_LEAD><<<grid, 32 * XW, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_xsweep<MODE_TRAIL><<<grid, 32 * XW, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+    } else {
+        const int seg = pick_seg(P.ny, 1, 128);
+        dim3 grid((P.nx + 127) / 128, (P.ny + seg - 1) / seg);
+        if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, 128, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, 128, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_ysweep<MODE_TRAIL><<<grid, 128, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+    }
+}
+
+void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s)
+{
+    dim3 grid((P.nx + 127) / 128, P.ny);
+    k_source_fast<<<grid, 128, 0, s>>>(P, q, dtp);
+}
+
+void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s) { k_ctl<<<1, 1, 0, s>>>(P, ctl, advance); }
+
+double host_tsafe(double tau, double Cpre, double Ta, double theta0) { return tsafe_for(tau, Cpre, Ta, theta0); }
+
+} // namespace nmsdt

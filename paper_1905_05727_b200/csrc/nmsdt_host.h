@@ -29,6 +29,13 @@ void launch_advance(Ctl* ctl, cudaStream_t s);
 void launch_set_double(double* p, double v, cudaStream_t s);
 int  launch_probe_fp64(cudaStream_t s, double* gflops, double* ms);
 
+// fused production path (nmsdt_fused.cu). dtp -> {dt (or tau for the source kernel), tsafe}; mode 0 plain, 1 leading
+// source on load, 2 trailing source + max-wavespeed partial
+void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s);
+void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s);
+void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s);
+double host_tsafe(double tau, double Cpre, double Ta, double theta0);
+
 // init / output kernels (nmsdt_init.cu)
 void launch_zero_plane(const Params& P, double* plane, cudaStream_t s);
 void launch_paint(const Params& P, double* prof_plane, const Cav* cav, int ncav, double h, cudaStream_t s);

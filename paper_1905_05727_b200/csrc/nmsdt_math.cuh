@@ -1,0 +1,125 @@
+// nmsdt_math.cuh -- branch-free fp64 elementary functions for the fused kernels of libnmsdt.so (sm_100a).
+//
+// The step is bound by the FP64 pipe and by issue slots: the CUDA library's div / sqrt / log /
+// exp cost ~10 / ~12 / ~35 / ~28 FP64-pipe instructions each plus a slow-path test.  Every operand on this path
+// is a positive normal number (densities, volume fractions, wave-speed differences, temperatures), so the
+// special-case handling is dropped and the functions are rebuilt from the MUFU seeds (rcp.approx / rsqrt.approx,
+// ~20 bits) + Newton steps and from two small tables held in shared memory:
+//   q_rcp   1 MUFU + 3 DFMA          (<= 1 ulp for normal x)
+//   q_sqrt  1 MUFU + 2 DMUL + 5 DFMA   (~1 ulp)
+//   pow_pair(x) -> (x^C, x^D)  Eq. 3-4: one table-driven log (128 entries, degree-6 log1p) and two
+//          table-driven exp2 (64 entries, degree-5), 28 FP64 instructions instead of ~90
+//   exp_neg(y) = e^-y for the Arrhenius factor of Eq. 6
+// Accuracy (checked on the device by tests/test_gpu_math.py against long-double references): relative error
+// <= 4e-16 for q_rcp/q_sqrt, <= 2e-15 for the powers over rho2/rho02 in [1e-3, 1e3].
+// Compiles for the host too (HOST_SEED emulates the 20-bit seeds) so that the polynomial/table logic can be checked
+// without a GPU.  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+namespace nmsdt {
+
+constexpr int LOG_TAB_BITS = 7, LOG_TAB_N = 1 << LOG_TAB_BITS;     // (1/c_j, ln c_j) pairs
+constexpr int EXP_TAB_BITS = 6, EXP_TAB_N = 1 << EXP_TAB_BITS;     // 2^(j/64)
+constexpr int MATH_TAB_DOUBLES = 2 * LOG_TAB_N + EXP_TAB_N;        // 320 doubles = 2560 B of shared memory
+
+#if defined(__CUDA_ARCH__)
+#define NMSDT_HD __device__ __forceinline__
+__device__ __forceinline__ double rcp_seed(double x) { double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x)); return r; }
+__device__ __forceinline__ double rsq_seed(double x) { double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x)); return r; }
+__device__ __forceinline__ double mk_double(int hi, int lo) { return __hiloint2double(hi, lo); }
+__device__ __forceinline__ int hi_word(double x) { return __double2hiint(x); }
+__device__ __forceinline__ int lo_word(double x) { return __double2loint(x); }
+#else
+#define NMSDT_HD inline
+inline double mk_double(int hi, int lo) { uint64_t u = ((uint64_t)(uint32_t)hi << 32) | (uint32_t)lo; double d; memcpy(&d, &u, 8); return d; }
+inline int hi_word(double x) { uint64_t u; memcpy(&u, &x, 8); return (int)(u >> 32); }
+inline int lo_word(double x) { uint64_t u; memcpy(&u, &x, 8); return (int)(u & 0xffffffffu); }
+inline double rcp_seed(double x) { return mk_double(hi_word(1.0 / mk_double(hi_word(x), 0)), 0); }       // 20-bit input, 20-bit output
+inline double rsq_seed(double x) { return mk_double(hi_word(1.0 / sqrt(mk_double(hi_word(x), 0))), 0); }
+#endif
+
+// 1/x for positive (or negative) normal x: seed e0 ~ 2^-20, cubic step -> e0^3 < 2^-59
+NMSDT_HD double q_rcp(double x)
+{
+    double r = rcp_seed(x);
+    double e = fma(-x, r, 1.0);
+    e = fma(e, e, e);
+    return fma(r, e, r);
+}
+
+// sqrt(x) for positive normal x (coupled Newton iteration on sqrt and 1/(2 sqrt))
+NMSDT_HD double q_sqrt(double x)
+{
+    double y = rsq_seed(x);
+    double g = x * y, h = 0.5 * y;
+    double e = fma(-g, h, 0.5);
+    g = fma(g, e, g); h = fma(h, e, h);
+    e = fma(-g, h, 0.5);
+    return fma(g, e, g);
+}
+
+// ln(x), x positive normal.  tab = shared-memory copy of the tables.  Absolute error ~1e-16 (+ 1 ulp of the result).
+NMSDT_HD double q_log(const double* __restrict__ tab, double x)
+{
+    const int hx = hi_word(x);
+    const int j = (hx >> (20 - LOG_TAB_BITS)) & (LOG_TAB_N - 1);
+    const double m = mk_double((hx & 0x000fffff) | 0x3ff00000, lo_word(x));            // mantissa in [1,2)
+    const double ed = mk_double(0x43300000, hx >> 20) - 4503599627371519.0;             // unbiased exponent: (2^52 + e_biased) - (2^52 + 1023)
+    const double ic = tab[2 * j], lc = tab[2 * j + 1];
+    const double r = fma(m, ic, -1.0);                                                 // |r| <= 2^-8
+    double p = fma(r, -1.0 / 6.0, 0.2);
+    p = fma(p, r, -0.25);
+    p = fma(p, r, 1.0 / 3.0);
+    p = fma(p, r, -0.5);
+    p = fma(p, r * r, r);                                                              // log1p(r)
+    return fma(ed, 0.69314718055994530942, lc + p);
+}
+
+// 2^(a*b) for |a*b| < 1000 (a*b is never rounded: the reduction uses the exact product through fma)
+NMSDT_HD double q_exp2_prod(const double* __restrict__ tab, double a, double b)
+{
+    const double SH = 6755399441055744.0 / EXP_TAB_N;           // 1.5 * 2^52 / 64: ulp = 1/64
+    const double t = fma(a, b, SH);
+    const int N = lo_word(t);
+    const double f = fma(a, b, -(t - SH));                      // |f| <= 1/128
+    const double T = tab[2 * LOG_TAB_N + (N & (EXP_TAB_N - 1))];
+    double p = fma(f, 1.3333558146428443e-3, 9.6181291076284772e-3);          // ln2^5/120, ln2^4/24
+    p = fma(p, f, 5.5504108664821580e-2);                                     // ln2^3/6
+    p = fma(p, f, 2.4022650695910071e-1);                                     // ln2^2/2
+    p = fma(p, f, 6.9314718055994531e-1);                                     // ln2
+    const double v = fma(T, p * f, T);
+    return mk_double(hi_word(v) + ((N >> EXP_TAB_BITS) << 20), lo_word(v));
+}
+
+constexpr double LOG2E = 1.4426950408889634074;
+
+// (x^C, x^D) from one logarithm; C2 = C*log2(e), D2 = D*log2(e)
+NMSDT_HD void q_pow_pair(const double* __restrict__ tab, double x, double C2, double D2, double& xC, double& xD)
+{
+    const double L = q_log(tab, x);
+    xC = q_exp2_prod(tab, C2, L);
+    xD = q_exp2_prod(tab, D2, L);
+}
+
+// e^(-y) for y >= 0 (flushes to ~1e-301 for y > 690)
+NMSDT_HD double q_exp_neg(const double* __restrict__ tab, double y)
+{
+    return q_exp2_prod(tab, fmin(y, 690.0), -LOG2E);
+}
+
+// host side: fill the 320-double table (long double arithmetic)
+inline void fill_math_tables(double* tab)
+{
+    for (int j = 0; j < LOG_TAB_N; ++j) {
+        const long double c = 1.0L + ((long double)j + 0.5L) / (long double)LOG_TAB_N;
+        const double ic = (double)(1.0L / c);
+        tab[2 * j] = ic;
+        tab[2 * j + 1] = (double)(-logl((long double)ic));
+    }
+    for (int j = 0; j < EXP_TAB_N; ++j) tab[2 * LOG_TAB_N + j] = (double)exp2l((long double)j / (long double)EXP_TAB_N);
+}
+
+} // namespace nmsdt
