@@ -30,7 +30,7 @@ struct FCell {            // W = (rho1, rho2, un, ut, p, z1, lambda) + what the 
 };
 struct FFace { double r1, r2, un, ut, p, z1, lam, rho, rhoE, c; };
 
-__device__ __forceinline__ double clampf(double x, double lo, double hi) { return fmin(fmax(x, lo), hi); }
+__device__ __forceinline__ double clampf(double x, double lo, double hi) { return dmin_(dmax_(x, lo), hi); }
 
 // R13 exact sub-step count (only reached by cells hotter than the safe bound; same exactly-rounded sequence as k_source)
 __device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
@@ -108,7 +108,7 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     W.p = p; W.lam = lam;
     const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
     const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22) * ixi;  // R10
-    W.rc2 = fmax(rc2, rho);                                                      // c^2 >= 1
+    W.rc2 = dmax_(rc2, rho);                                                      // c^2 >= 1
 }
 
 __device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f)
@@ -127,7 +127,7 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
     const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22);
-    f.c = q_sqrt(fmax(rc2 * q_rcp(xi * rho), 1.0));
+    f.c = q_sqrt(dmax_(rc2 * q_rcp(xi * rho), 1.0));
 }
 
 __device__ __forceinline__ double limited_f(int kind, double a, double b)
@@ -135,7 +135,7 @@ __device__ __forceinline__ double limited_f(int kind, double a, double b)
     const double ab = a * b;
     double m;
     if (kind == 0) m = fabs(a) < fabs(b) ? a : b;                                 // minmod (R5)
-    else { m = fmin(fmin(2.0 * fabs(a), 2.0 * fabs(b)), 0.5 * fabs(a + b)); m = a > 0.0 ? m : -m; }
+    else { m = dmin_(dmin_(2.0 * fabs(a), 2.0 * fabs(b)), 0.5 * fabs(a + b)); m = a > 0.0 ? m : -m; }
     return ab > 0.0 ? m : 0.0;
 }
 
@@ -174,8 +174,8 @@ __device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, con
 // O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
 __device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double F[8])
 {
-    const double SL = fmin(L.un - L.c, R.un - R.c);                  // R9: Davis
-    const double SR = fmax(L.un + L.c, R.un + R.c);
+    const double SL = dmin_(L.un - L.c, R.un - R.c);                  // R9: Davis
+    const double SR = dmax_(L.un + L.c, R.un + R.c);
     const double mL = L.rho * (SL - L.un), mR = R.rho * (SR - R.un);
     const double Sstar = (R.p - L.p + fma(L.un, mL, -R.un * mR)) * q_rcp(mL - mR);
     const bool useL = (SL >= 0.0) || ((SR > 0.0) && (Sstar >= 0.0));
@@ -218,10 +218,10 @@ __device__ __forceinline__ void trail_cell(const Params& P, const double* __rest
     FCell W; double dE, q6n;
     prim_cell<true>(P, tab, o, tau, Tsafe, W, dE, q6n);
     o[4] += dE; o[6] = q6n;
-    const double a = fmax(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
+    const double a = dmax_(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
     const bool ok = all_finite7(o) && o[0] > 0.0 && o[1] > 0.0 && (__double2hiint(a) & 0x7fffffff) < 0x7ff00000;
     bad |= ok ? 0 : 1;
-    smax = fmax(smax, a);
+    smax = dmax_(smax, a);
 }
 
 __device__ __forceinline__ void reduce_smax(double smax, int bad, Ctl* ctl)
@@ -249,38 +249,77 @@ __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double la
 constexpr int XW = 4;                       // warps per block in k_xsweep
 constexpr int RING = 33;
 constexpr int RING_DOUBLES = (16 + 10 + 8) * RING;
+constexpr int PRING = 66;                   // staged input pairs: chunk k (32 slots), chunk k+1 in flight, lane 31 of chunk k-1
+constexpr int XS_DOUBLES = MATH_TAB_DOUBLES + XW * (RING_DOUBLES + 7 * PRING * 2);
 
 } // namespace
 
 // ---------------------------------------------------------------------------------------------------------------
 // y-sweep (a5): thread per column, register marching
 // ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async8(double* smem, const double* gmem)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async16(double* smem, const double* gmem)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int YT = 128;      // threads (columns) per block in k_ysweep
+constexpr int YST = 4;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1, c+2 in flight
+
 template <int MODE>
-__global__ void __launch_bounds__(128) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
-                                                const double* __restrict__ dtp, Ctl* ctl, int seg)
+__global__ void __launch_bounds__(YT, 3) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
+                                               const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
     __shared__ double s_tab[MATH_TAB_DOUBLES];
+    __shared__ double s_q[YST][7][YT];           // thread-private slots: no barrier, only cp.async.wait_group
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    const int tid = threadIdx.x;
+    const int col = blockIdx.x * YT + tid;
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
         const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
         const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
         const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
         const long long fs = P.fstride, pitch = P.pitch;
-        const double* pin = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
+        // field order of the sweep: normal momentum = q3, tangential = q2
+        const double* gp[7];
+        {
+            const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
+            gp[0] = g; gp[1] = g + fs; gp[2] = g + 3 * fs; gp[3] = g + 2 * fs; gp[4] = g + 4 * fs; gp[5] = g + 5 * fs; gp[6] = g + 6 * fs;
+        }
         double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
+        const int nrows = c1 - c0 + 4;
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+#pragma unroll
+            for (int k = 0; k < 7; ++k) { cp_async8(&s_q[r][k][tid], gp[k]); gp[k] += pitch; }
+            cp_async_commit();
+        }
         FCell Wm, W0, Wp;
         Wm = W0 = FCell{1, 1, 0, 0, 1, 0.5, 0, 1, 1};
         FFace prevR = FFace{1, 1, 0, 0, 1, 0.5, 0, 1, 1, 1};
         double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
-        for (int c = c0 - 2; c < c1 + 2; ++c, pin += pitch) {
+        for (int jj = 0; jj < nrows; ++jj) {         // row c = c0 - 2 + jj
+            if (jj + 2 < nrows) {
+#pragma unroll
+                for (int k = 0; k < 7; ++k) { cp_async8(&s_q[(jj + 2) & (YST - 1)][k][tid], gp[k]); gp[k] += pitch; }
+            }
+            cp_async_commit();
+            cp_async_wait<2>();
             double q[7];
-            q[0] = pin[0]; q[1] = pin[fs]; q[2] = pin[3 * fs]; q[3] = pin[2 * fs]; q[4] = pin[4 * fs]; q[5] = pin[5 * fs]; q[6] = pin[6 * fs];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) q[k] = s_q[jj & (YST - 1)][k][tid];
             double dE, q6n;
             prim_cell<MODE == MODE_LEAD>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n);
-            const int jj = c - (c0 - 2);
             if (jj >= 2) {                       // centre cell c-1 has both neighbours
                 double WL[7], WR[7];
                 recon_fast(P, Wm, W0, Wp, khalf, WL, WR);
@@ -300,10 +339,10 @@ __global__ void __launch_bounds__(128) k_ysweep(const __grid_constant__ Params P
                         pout[6 * fs] = o[6];
                         pout += pitch;
                     }
-                    if (c - 1 < c1) {            // start cell c-1 with its lower-face flux
-                        const double* pc = pin - pitch;
+                    if (jj < nrows - 1) {        // start cell c-1 (< c1) with its lower-face flux
                         double o[7];
-                        o[0] = pc[0]; o[1] = pc[fs]; o[2] = pc[3 * fs]; o[3] = pc[2 * fs]; o[4] = pc[4 * fs]; o[5] = pc[5 * fs]; o[6] = pc[6 * fs];
+#pragma unroll
+                        for (int k = 0; k < 7; ++k) o[k] = s_q[(jj - 1) & (YST - 1)][k][tid];
                         if (MODE == MODE_LEAD) lead_fix(P, o, W0.lam);
                         z1n = o[5];
 #pragma unroll
@@ -315,6 +354,7 @@ __global__ void __launch_bounds__(128) k_ysweep(const __grid_constant__ Params P
             }
             Wm = W0; W0 = Wp;
         }
+        cp_async_wait<0>();
     }
     if (MODE == MODE_TRAIL) reduce_smax(smax, bad, ctl);
 }
@@ -326,8 +366,9 @@ template <int MODE>
 __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
                                                     const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
-    __shared__ double s_tab[MATH_TAB_DOUBLES];
-    __shared__ double s_ring[XW * RING_DOUBLES];
+    extern __shared__ __align__(16) double s_dyn[];
+    double* s_tab = s_dyn;
+    double* s_ring = s_dyn + MATH_TAB_DOUBLES;
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -337,6 +378,7 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
         double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
         double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
         double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
+        double2* stg = reinterpret_cast<double2*>(s_dyn + MATH_TAB_DOUBLES + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
         const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
         const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
         const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
@@ -347,19 +389,33 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
         const int niter = (c1 - c0 + 63) >> 6;
         const bool fixed_in = (MODE == MODE_LEAD) && (P.bc_xlo == 3);
         int sw = lane;                                   // ring slot written by this lane: (32 k + lane) mod 33
+        int ps = lane;                                   // staging slot of this lane's pair: (32 k + lane) mod 66
+        {   // stage chunk 0 (cells c0-62 .. c0+1; only lanes 30, 31 are used)
+            const int Ac = min(max(c0 - 64 + 2 * lane + 2, -2), nxe);
+#pragma unroll
+            for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + ps), rin + Ac + f * fs);
+            cp_async_commit();
+        }
         for (int k = 0; k <= niter; ++k) {
             const int b = c0 + 64 * (k - 1);             // first cell updated in this iteration
             const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
             const bool act = (k > 0) || (lane >= 30);    // iteration 0 only primes the rings (cells c0-2 .. c0+1)
             const int sr = sw == 0 ? RING - 1 : sw - 1;  // left neighbour's slot
             FCell WA, WB;
-            // ---- phase 1: load, primitives (+ leading source) ----------------------------------------------------
+            const int psn = ps + 32 >= PRING ? ps + 32 - PRING : ps + 32;
+            if (k < niter) {                             // stage the next chunk while this one is computed
+                const int An = min(A + 64, nxe);
+#pragma unroll
+                for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + psn), rin + An + f * fs);
+            }
+            cp_async_commit();
+            cp_async_wait<1>();
+            // ---- phase 1: primitives (+ leading source) of the staged pair -----------------------------------------
             if (act) {
                 const int Ac = min(A, nxe);
-                const double* pa = rin + Ac;
                 double qa[7], qb[7];
 #pragma unroll
-                for (int f = 0; f < 7; ++f) { const double2 v = *reinterpret_cast<const double2*>(pa + f * fs); qa[f] = v.x; qb[f] = v.y; }
+                for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
                 double dE, q6n;
                 prim_cell<MODE == MODE_LEAD>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n);
                 prim_cell<MODE == MODE_LEAD>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n);
@@ -413,10 +469,10 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
                 double F0[8];
 #pragma unroll
                 for (int f = 0; f < 8; ++f) F0[f] = rf[f * RING + sr];
-                const double* pu = rin + u0;
+                const int pl = ps == 0 ? PRING - 1 : ps - 1;      // the pair staged by the left neighbour = cells u0, u0+1
                 double oa[7], ob[7];
 #pragma unroll
-                for (int f = 0; f < 7; ++f) { const double2 v = *reinterpret_cast<const double2*>(pu + f * fs); oa[f] = v.x; ob[f] = v.y; }
+                for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + pl]; oa[f] = v.x; ob[f] = v.y; }
                 if (MODE == MODE_LEAD) {
                     lead_fix(P, oa, lam_u0);
                     lead_fix(P, ob, lam_u1);
@@ -443,7 +499,9 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
                 }
             }
             sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
+            ps = psn;
         }
+        cp_async_wait<0>();
     }
     if (MODE == MODE_TRAIL) reduce_smax(smax, bad, ctl);
 }
@@ -514,15 +572,23 @@ void launch_sweep_fused(const Params& P, const double* qin, double* qout, const 
     if (dir == 0) {
         const int seg = pick_seg(P.nx, 64, 2048);
         dim3 grid((P.ny + XW - 1) / XW, (P.nx + seg - 1) / seg);
-        if (mode == MODE_PLAIN)      k_xsweep<MODE_PLAIN><<<grid, 32 * XW, 0, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_LEAD)  k_xsweep<MODE_LEAD><<<grid, 32 * XW, 0, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_xsweep<MODE_TRAIL><<<grid, 32 * XW, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        const size_t sm = XS_DOUBLES * sizeof(double);
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaFuncSetAttribute(k_xsweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            cudaFuncSetAttribute(k_xsweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            cudaFuncSetAttribute(k_xsweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            attr_done = true;
+        }
+        if (mode == MODE_PLAIN)      k_xsweep<MODE_PLAIN><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_LEAD)  k_xsweep<MODE_LEAD><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_xsweep<MODE_TRAIL><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
     } else {
         const int seg = pick_seg(P.ny, 1, 128);
-        dim3 grid((P.nx + 127) / 128, (P.ny + seg - 1) / seg);
-        if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, 128, 0, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, 128, 0, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_ysweep<MODE_TRAIL><<<grid, 128, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        dim3 grid((P.nx + YT - 1) / YT, (P.ny + seg - 1) / seg);
+        if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, YT, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, YT, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_ysweep<MODE_TRAIL><<<grid, YT, 0, s>>>(P, qin, qout, dtp, ctl, seg);
     }
 }
 

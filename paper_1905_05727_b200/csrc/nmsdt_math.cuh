@@ -41,6 +41,23 @@ inline double rcp_seed(double x) { return mk_double(hi_word(1.0 / mk_double(hi_w
 inline double rsq_seed(double x) { return mk_double(hi_word(1.0 / sqrt(mk_double(hi_word(x), 0))), 0); }
 #endif
 
+// polynomial coefficients: kept in the constant bank on the device so that DFMA reads them as c[][] operands
+// (as 64-bit immediates each costs two moves per use)
+#if defined(__CUDACC__)
+#define NMSDT_KCONST static __constant__ double
+#else
+#define NMSDT_KCONST static const double
+#endif
+NMSDT_KCONST KC[10] = {
+    -1.0 / 6.0, 0.2, 1.0 / 3.0, 0.69314718055994530942,                                  // log1p series, ln 2
+    1.3333558146428443e-3, 9.6181291076284772e-3, 5.5504108664821580e-2,                 // ln2^5/120, ln2^4/24, ln2^3/6
+    2.4022650695910071e-1, 6.9314718055994531e-1, 1.4426950408889634074};                // ln2^2/2, ln2, log2(e)
+
+// min / max without the NaN rules of fmin / fmax (3 instructions instead of 5-6; operands here are never NaN on a
+// valid state, and an invalid state is caught on the conserved variables)
+NMSDT_HD double dmin_(double a, double b) { return a < b ? a : b; }
+NMSDT_HD double dmax_(double a, double b) { return a > b ? a : b; }
+
 // 1/x for positive (or negative) normal x: seed e0 ~ 2^-20, cubic step -> e0^3 < 2^-59
 NMSDT_HD double q_rcp(double x)
 {
@@ -70,12 +87,12 @@ NMSDT_HD double q_log(const double* __restrict__ tab, double x)
     const double ed = mk_double(0x43300000, hx >> 20) - 4503599627371519.0;             // unbiased exponent: (2^52 + e_biased) - (2^52 + 1023)
     const double ic = tab[2 * j], lc = tab[2 * j + 1];
     const double r = fma(m, ic, -1.0);                                                 // |r| <= 2^-8
-    double p = fma(r, -1.0 / 6.0, 0.2);
+    double p = fma(r, KC[0], KC[1]);
     p = fma(p, r, -0.25);
-    p = fma(p, r, 1.0 / 3.0);
+    p = fma(p, r, KC[2]);
     p = fma(p, r, -0.5);
     p = fma(p, r * r, r);                                                              // log1p(r)
-    return fma(ed, 0.69314718055994530942, lc + p);
+    return fma(ed, KC[3], lc + p);
 }
 
 // 2^(a*b) for |a*b| < 1000 (a*b is never rounded: the reduction uses the exact product through fma)
@@ -86,10 +103,10 @@ NMSDT_HD double q_exp2_prod(const double* __restrict__ tab, double a, double b)
     const int N = lo_word(t);
     const double f = fma(a, b, -(t - SH));                      // |f| <= 1/128
     const double T = tab[2 * LOG_TAB_N + (N & (EXP_TAB_N - 1))];
-    double p = fma(f, 1.3333558146428443e-3, 9.6181291076284772e-3);          // ln2^5/120, ln2^4/24
-    p = fma(p, f, 5.5504108664821580e-2);                                     // ln2^3/6
-    p = fma(p, f, 2.4022650695910071e-1);                                     // ln2^2/2
-    p = fma(p, f, 6.9314718055994531e-1);                                     // ln2
+    double p = fma(f, KC[4], KC[5]);
+    p = fma(p, f, KC[6]);
+    p = fma(p, f, KC[7]);
+    p = fma(p, f, KC[8]);
     const double v = fma(T, p * f, T);
     return mk_double(hi_word(v) + ((N >> EXP_TAB_BITS) << 20), lo_word(v));
 }
@@ -107,7 +124,7 @@ NMSDT_HD void q_pow_pair(const double* __restrict__ tab, double x, double C2, do
 // e^(-y) for y >= 0 (flushes to ~1e-301 for y > 690)
 NMSDT_HD double q_exp_neg(const double* __restrict__ tab, double y)
 {
-    return q_exp2_prod(tab, fmin(y, 690.0), -LOG2E);
+    return q_exp2_prod(tab, dmin_(y, 690.0), -KC[9]);
 }
 
 // host side: fill the 320-double table (long double arithmetic)
