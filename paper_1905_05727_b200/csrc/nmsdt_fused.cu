@@ -132,11 +132,14 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
 
 __device__ __forceinline__ double limited_f(int kind, double a, double b)
 {
-    const double ab = a * b;
-    double m;
-    if (kind == 0) m = fabs(a) < fabs(b) ? a : b;                                 // minmod (R5)
-    else { m = dmin_(dmin_(2.0 * fabs(a), 2.0 * fabs(b)), 0.5 * fabs(a + b)); m = a > 0.0 ? m : -m; }
-    return ab > 0.0 ? m : 0.0;
+    if (kind == 0) {                                                              // minmod (R5)
+        // a b > 0 <=> equal sign bits and both non-zero; if either is zero the smaller magnitude is that zero
+        const double m = fabs(a) < fabs(b) ? a : b;
+        return ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
+    }
+    double m = dmin_(dmin_(2.0 * fabs(a), 2.0 * fabs(b)), 0.5 * fabs(a + b));     // monotonised central
+    m = a > 0.0 ? m : -m;
+    return a * b > 0.0 ? m : 0.0;
 }
 
 // O4.1-2 for the centre cell W0
@@ -183,24 +186,24 @@ __device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double
     const double r1 = useL ? L.r1 : R.r1, r2 = useL ? L.r2 : R.r2, un = useL ? L.un : R.un, ut = useL ? L.ut : R.ut;
     const double p = useL ? L.p : R.p, z1 = useL ? L.z1 : R.z1, lam = useL ? L.lam : R.lam;
     const double rho = useL ? L.rho : R.rho, rhoE = useL ? L.rhoE : R.rhoE, SK = useL ? SL : SR;
-    double U[7], FK[7];
-    U[0] = z1 * r1; U[1] = (1.0 - z1) * r2; U[2] = rho * un; U[3] = rho * ut; U[4] = rhoE; U[5] = z1; U[6] = U[1] * lam;
-    FK[0] = U[0] * un; FK[1] = U[1] * un; FK[2] = fma(U[2], un, p); FK[3] = U[2] * ut; FK[4] = (rhoE + p) * un;
-    FK[5] = z1 * un; FK[6] = U[6] * un;
-    // chi = (SK-un)/(SK-S*), p/(SK-un) from one reciprocal
+    // chi = (SK-un)/(SK-S*) and p/(SK-un) from one reciprocal; outside the fan SKs = 0 and the star terms vanish
     const double a = SK - un, b = SK - Sstar;
-    const double rab = star ? q_rcp(a * b) : 0.0;                     // keeps the unused star state finite outside the fan
+    const double rab = star ? q_rcp(a * b) : 0.0;
     const double chi = a * a * rab;
     const double poa = p * b * rab;
-    double Us[7];
-#pragma unroll
-    for (int k = 0; k < 7; ++k) Us[k] = chi * U[k];
-    Us[2] = rho * chi * Sstar;
-    Us[4] = chi * fma(Sstar - un, fma(rho, Sstar, poa), rhoE);
-    const double SKs = star ? SK : 0.0;                               // F = FK + SK (U* - U) in the star region, FK otherwise
-#pragma unroll
-    for (int k = 0; k < 7; ++k) F[k] = fma(SKs, Us[k] - U[k], FK[k]);
-    F[7] = fma(SKs, chi - 1.0, un);
+    const double SKs = star ? SK : 0.0;
+    // U*_k = chi U_k for the advected components, so F_k = U_k un + SK (chi - 1) U_k = U_k u_face with the
+    // HLLC-consistent face velocity u_face = un + SK (chi - 1) (R8)
+    const double uf = fma(SKs, chi - 1.0, un);
+    const double U0 = z1 * r1, U1 = (1.0 - z1) * r2;
+    F[0] = U0 * uf;
+    F[1] = U1 * uf;
+    F[2] = fma(rho * un, un, p) + SKs * rho * fma(chi, Sstar, -un);
+    F[3] = rho * ut * uf;
+    F[4] = fma(rhoE + p, un, SKs * fma(chi, fma(Sstar - un, fma(rho, Sstar, poa), rhoE), -rhoE));
+    F[5] = z1 * uf;
+    F[6] = U1 * lam * uf;
+    F[7] = uf;
 }
 
 __device__ __forceinline__ bool all_finite7(const double o[7])
@@ -246,6 +249,12 @@ __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double la
     }
 }
 
+#ifndef NMSDT_Y_MINBLOCKS
+#define NMSDT_Y_MINBLOCKS 4
+#endif
+#ifndef NMSDT_X_MINBLOCKS
+#define NMSDT_X_MINBLOCKS 2
+#endif
 constexpr int XW = 4;                       // warps per block in k_xsweep
 constexpr int RING = 33;
 constexpr int RING_DOUBLES = (16 + 10 + 8) * RING;
@@ -272,14 +281,21 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 constexpr int YT = 128;      // threads (columns) per block in k_ysweep
-constexpr int YST = 4;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1, c+2 in flight
+constexpr int YST = 3;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1 in flight
+constexpr int YS_DOUBLES = MATH_TAB_DOUBLES + (YST * 7 + 2 * 9 + 10) * YT;
 
+// Per-thread state that lives across rows is kept in thread-private shared-memory slots ([..][YT] layout, conflict
+// free, no barriers): the staged input rows, the primitive window (cells c-2, c-1) and the previous right-face state.
+// Only the half-finished update of cell c-1 stays in registers; this keeps the kernel at 128 registers (16 warps/SM).
 template <int MODE>
-__global__ void __launch_bounds__(YT, 3) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
-                                               const double* __restrict__ dtp, Ctl* ctl, int seg)
+__global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin,
+                                                                  double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
-    __shared__ double s_tab[MATH_TAB_DOUBLES];
-    __shared__ double s_q[YST][7][YT];           // thread-private slots: no barrier, only cp.async.wait_group
+    extern __shared__ __align__(16) double s_dyn[];
+    double* s_tab = s_dyn;
+    double (*s_q)[7][YT] = reinterpret_cast<double (*)[7][YT]>(s_dyn + MATH_TAB_DOUBLES);
+    double (*s_w)[9][YT] = reinterpret_cast<double (*)[9][YT]>(s_dyn + MATH_TAB_DOUBLES + YST * 7 * YT);
+    double (*s_r)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + MATH_TAB_DOUBLES + (YST * 7 + 2 * 9) * YT);
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int tid = threadIdx.x;
@@ -291,68 +307,88 @@ __global__ void __launch_bounds__(YT, 3) k_ysweep(const __grid_constant__ Params
         const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
         const long long fs = P.fstride, pitch = P.pitch;
         // field order of the sweep: normal momentum = q3, tangential = q2
-        const double* gp[7];
-        {
-            const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
-            gp[0] = g; gp[1] = g + fs; gp[2] = g + 3 * fs; gp[3] = g + 2 * fs; gp[4] = g + 4 * fs; gp[5] = g + 5 * fs; gp[6] = g + 6 * fs;
-        }
+        const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
         double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
         const int nrows = c1 - c0 + 4;
-#pragma unroll
-        for (int r = 0; r < 2; ++r) {
-#pragma unroll
-            for (int k = 0; k < 7; ++k) { cp_async8(&s_q[r][k][tid], gp[k]); gp[k] += pitch; }
-            cp_async_commit();
-        }
-        FCell Wm, W0, Wp;
-        Wm = W0 = FCell{1, 1, 0, 0, 1, 0.5, 0, 1, 1};
-        FFace prevR = FFace{1, 1, 0, 0, 1, 0.5, 0, 1, 1, 1};
+        cp_async8(&s_q[0][0][tid], g); cp_async8(&s_q[0][1][tid], g + fs); cp_async8(&s_q[0][2][tid], g + 3 * fs);
+        cp_async8(&s_q[0][3][tid], g + 2 * fs); cp_async8(&s_q[0][4][tid], g + 4 * fs); cp_async8(&s_q[0][5][tid], g + 5 * fs);
+        cp_async8(&s_q[0][6][tid], g + 6 * fs);
+        cp_async_commit();
+        g += pitch;
         double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
-        for (int jj = 0; jj < nrows; ++jj) {         // row c = c0 - 2 + jj
-            if (jj + 2 < nrows) {
-#pragma unroll
-                for (int k = 0; k < 7; ++k) { cp_async8(&s_q[(jj + 2) & (YST - 1)][k][tid], gp[k]); gp[k] += pitch; }
+        int st = 0;                                   // stage of row jj (jj mod 3)
+        for (int jj = 0; jj < nrows; ++jj) {          // row c = c0 - 2 + jj
+            const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
+            if (jj + 1 < nrows) {
+                cp_async8(&s_q[sn][0][tid], g); cp_async8(&s_q[sn][1][tid], g + fs); cp_async8(&s_q[sn][2][tid], g + 3 * fs);
+                cp_async8(&s_q[sn][3][tid], g + 2 * fs); cp_async8(&s_q[sn][4][tid], g + 4 * fs); cp_async8(&s_q[sn][5][tid], g + 5 * fs);
+                cp_async8(&s_q[sn][6][tid], g + 6 * fs);
+                g += pitch;
             }
             cp_async_commit();
-            cp_async_wait<2>();
-            double q[7];
+            cp_async_wait<1>();
+            FCell Wp;
+            {
+                double q[7];
 #pragma unroll
-            for (int k = 0; k < 7; ++k) q[k] = s_q[jj & (YST - 1)][k][tid];
-            double dE, q6n;
-            prim_cell<MODE == MODE_LEAD>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n);
-            if (jj >= 2) {                       // centre cell c-1 has both neighbours
-                double WL[7], WR[7];
-                recon_fast(P, Wm, W0, Wp, khalf, WL, WR);
-                if (jj >= 3) {
-                    FFace fl;
-                    face_fast(P, s_tab, WL, fl);
-                    double F[8];
-                    hllc_fast(prevR, fl, F);     // face between cells c-2 and c-1
-                    if (jj >= 4) {               // finish cell c-2
-                        double o[7];
-#pragma unroll
-                        for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
-                        o[5] = fma(dtdx * z1n, F[7], o[5]);                       // R8: non-conservative z1 term
-                        o[5] = clampf(o[5], P.z_min, P.z_max);
-                        if (MODE == MODE_TRAIL) trail_cell(P, s_tab, o, tau, Tsafe, smax, bad);
-                        pout[0] = o[0]; pout[fs] = o[1]; pout[3 * fs] = o[2]; pout[2 * fs] = o[3]; pout[4 * fs] = o[4]; pout[5 * fs] = o[5];
-                        pout[6 * fs] = o[6];
-                        pout += pitch;
-                    }
-                    if (jj < nrows - 1) {        // start cell c-1 (< c1) with its lower-face flux
-                        double o[7];
-#pragma unroll
-                        for (int k = 0; k < 7; ++k) o[k] = s_q[(jj - 1) & (YST - 1)][k][tid];
-                        if (MODE == MODE_LEAD) lead_fix(P, o, W0.lam);
-                        z1n = o[5];
-#pragma unroll
-                        for (int k = 0; k < 7; ++k) acc[k] = fma(dtdx, F[k], o[k]);
-                        acc[5] = fma(-dtdx * z1n, F[7], acc[5]);
-                    }
-                }
-                face_fast(P, s_tab, WR, prevR);
+                for (int k = 0; k < 7; ++k) q[k] = s_q[st][k][tid];
+                double dE, q6n;
+                prim_cell<MODE == MODE_LEAD>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n);
             }
-            Wm = W0; W0 = Wp;
+            // The body is branch free: during the 4 ramp-up rows it runs on not-yet-valid window / face / flux values
+            // (finite or not, never stored: the store and the wavespeed contribution are predicated on jj >= 4).
+            const int wm = jj & 1, w0 = wm ^ 1;       // window slots of cells c-2 and c-1
+            double WL[7], WR[7], lam0c;
+            {                                         // centre cell c-1
+                FCell Wm, W0;
+                Wm.r1 = s_w[wm][0][tid]; Wm.r2 = s_w[wm][1][tid]; Wm.un = s_w[wm][2][tid]; Wm.ut = s_w[wm][3][tid]; Wm.p = s_w[wm][4][tid];
+                Wm.z1 = s_w[wm][5][tid]; Wm.lam = s_w[wm][6][tid]; Wm.irho = 0.0; Wm.rc2 = 0.0;
+                W0.r1 = s_w[w0][0][tid]; W0.r2 = s_w[w0][1][tid]; W0.un = s_w[w0][2][tid]; W0.ut = s_w[w0][3][tid]; W0.p = s_w[w0][4][tid];
+                W0.z1 = s_w[w0][5][tid]; W0.lam = s_w[w0][6][tid]; W0.irho = s_w[w0][7][tid]; W0.rc2 = s_w[w0][8][tid];
+                lam0c = W0.lam;
+                recon_fast(P, Wm, W0, Wp, khalf, WL, WR);
+            }
+            s_w[wm][0][tid] = Wp.r1; s_w[wm][1][tid] = Wp.r2; s_w[wm][2][tid] = Wp.un; s_w[wm][3][tid] = Wp.ut; s_w[wm][4][tid] = Wp.p;
+            s_w[wm][5][tid] = Wp.z1; s_w[wm][6][tid] = Wp.lam; s_w[wm][7][tid] = Wp.irho; s_w[wm][8][tid] = Wp.rc2;
+            FFace fl, fr, pr;
+            face_fast(P, s_tab, WL, fl);
+            face_fast(P, s_tab, WR, fr);
+            pr.r1 = s_r[0][tid]; pr.r2 = s_r[1][tid]; pr.un = s_r[2][tid]; pr.ut = s_r[3][tid]; pr.p = s_r[4][tid];
+            pr.z1 = s_r[5][tid]; pr.lam = s_r[6][tid]; pr.rho = s_r[7][tid]; pr.rhoE = s_r[8][tid]; pr.c = s_r[9][tid];
+            s_r[0][tid] = fr.r1; s_r[1][tid] = fr.r2; s_r[2][tid] = fr.un; s_r[3][tid] = fr.ut; s_r[4][tid] = fr.p;
+            s_r[5][tid] = fr.z1; s_r[6][tid] = fr.lam; s_r[7][tid] = fr.rho; s_r[8][tid] = fr.rhoE; s_r[9][tid] = fr.c;
+            double F[8];
+            hllc_fast(pr, fl, F);                     // face between cells c-2 and c-1
+            {                                         // finish cell c-2
+                double o[7];
+#pragma unroll
+                for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
+                o[5] = fma(dtdx * z1n, F[7], o[5]);                           // R8: non-conservative z1 term
+                o[5] = clampf(o[5], P.z_min, P.z_max);
+                const bool valid = jj >= 4;
+                if (MODE == MODE_TRAIL) {
+                    double sm1 = 0.0; int bad1 = 0;
+                    trail_cell(P, s_tab, o, tau, Tsafe, sm1, bad1);
+                    smax = valid ? dmax_(smax, sm1) : smax;
+                    bad |= valid ? bad1 : 0;
+                }
+                if (valid) {
+                    pout[0] = o[0]; pout[fs] = o[1]; pout[3 * fs] = o[2]; pout[2 * fs] = o[3]; pout[4 * fs] = o[4]; pout[5 * fs] = o[5];
+                    pout[6 * fs] = o[6];
+                    pout += pitch;
+                }
+            }
+            {                                         // start cell c-1 with its lower-face flux
+                double o[7];
+#pragma unroll
+                for (int k = 0; k < 7; ++k) o[k] = s_q[sp][k][tid];
+                if (MODE == MODE_LEAD) lead_fix(P, o, lam0c);
+                z1n = o[5];
+#pragma unroll
+                for (int k = 0; k < 7; ++k) acc[k] = fma(dtdx, F[k], o[k]);
+                acc[5] = fma(-dtdx * z1n, F[7], acc[5]);
+            }
+            st = sn;
         }
         cp_async_wait<0>();
     }
@@ -363,7 +399,7 @@ __global__ void __launch_bounds__(YT, 3) k_ysweep(const __grid_constant__ Params
 // x-sweep (a4): warp per row segment, 2 cells per lane, shared-memory rings between lanes
 // ---------------------------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
+__global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
                                                     const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
     extern __shared__ __align__(16) double s_dyn[];
@@ -399,7 +435,8 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
         for (int k = 0; k <= niter; ++k) {
             const int b = c0 + 64 * (k - 1);             // first cell updated in this iteration
             const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
-            const bool act = (k > 0) || (lane >= 30);    // iteration 0 only primes the rings (cells c0-2 .. c0+1)
+            // iteration 0 only primes the rings (cells c0-2 .. c0+1 through lanes 30, 31); the body is branch free and
+            // simply runs on clamped / not-yet-valid data there, nothing of which is stored
             const int sr = sw == 0 ? RING - 1 : sw - 1;  // left neighbour's slot
             FCell WA, WB;
             const int psn = ps + 32 >= PRING ? ps + 32 - PRING : ps + 32;
@@ -411,8 +448,8 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
             cp_async_commit();
             cp_async_wait<1>();
             // ---- phase 1: primitives (+ leading source) of the staged pair -----------------------------------------
-            if (act) {
-                const int Ac = min(A, nxe);
+            {
+                const int Ac = min(max(A, -2), nxe);
                 double qa[7], qb[7];
 #pragma unroll
                 for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
@@ -429,7 +466,7 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
             // ---- phase 2: reconstruct cells A-1 and A, four face states ------------------------------------------
             FFace FL1, FR1, FL2;
             double lam_u0 = 0.0, lam_u1 = 0.0;
-            if (act) {
+            {
                 FCell Wmm, Wm1;
                 Wmm.r1 = rw[0 * RING + sr]; Wmm.r2 = rw[1 * RING + sr]; Wmm.un = rw[2 * RING + sr]; Wmm.ut = rw[3 * RING + sr];
                 Wmm.p = rw[4 * RING + sr];  Wmm.z1 = rw[5 * RING + sr]; Wmm.lam = rw[6 * RING + sr]; Wmm.irho = 0.0; Wmm.rc2 = 0.0;
@@ -452,7 +489,7 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
             __syncwarp();
             // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
             double F1[8], F2[8];
-            if (act) {
+            {
                 FFace FRp;
                 FRp.r1 = rfr[0 * RING + sr]; FRp.r2 = rfr[1 * RING + sr]; FRp.un = rfr[2 * RING + sr]; FRp.ut = rfr[3 * RING + sr];
                 FRp.p = rfr[4 * RING + sr];  FRp.z1 = rfr[5 * RING + sr]; FRp.lam = rfr[6 * RING + sr]; FRp.rho = rfr[7 * RING + sr];
@@ -465,7 +502,8 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
             __syncwarp();
             // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
             const int u0 = b + 2 * lane;
-            if (k > 0 && u0 < c1) {
+            {
+                const bool valid = k > 0 && u0 < c1;
                 double F0[8];
 #pragma unroll
                 for (int f = 0; f < 8; ++f) F0[f] = rf[f * RING + sr];
@@ -484,18 +522,22 @@ __global__ void __launch_bounds__(32 * XW) k_xsweep(const __grid_constant__ Para
                 ob[5] = clampf(fma(dtdx * zb, F2[7] - F1[7], ob[5]), P.z_min, P.z_max);
                 const bool two = u0 + 1 < c1;
                 if (MODE == MODE_TRAIL) {
-                    trail_cell(P, s_tab, oa, tau, Tsafe, smax, bad);
-                    double sm2 = 0.0; int bad2 = 0;
+                    double sm1 = 0.0, sm2 = 0.0; int bad1 = 0, bad2 = 0;
+                    trail_cell(P, s_tab, oa, tau, Tsafe, sm1, bad1);
                     trail_cell(P, s_tab, ob, tau, Tsafe, sm2, bad2);
-                    if (two) { smax = fmax(smax, sm2); bad |= bad2; }
+                    sm1 = valid ? sm1 : 0.0; sm2 = (valid && two) ? sm2 : 0.0;
+                    smax = dmax_(smax, dmax_(sm1, sm2));
+                    bad |= (valid ? bad1 : 0) | ((valid && two) ? bad2 : 0);
                 }
                 double* po = rout + u0;
-                if (two) {
+                if (valid) {
+                    if (two) {
 #pragma unroll
-                    for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
-                } else {
+                        for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
+                    } else {
 #pragma unroll
-                    for (int f = 0; f < 7; ++f) po[f * fs] = oa[f];
+                        for (int f = 0; f < 7; ++f) po[f * fs] = oa[f];
+                    }
                 }
             }
             sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
@@ -586,9 +628,17 @@ void launch_sweep_fused(const Params& P, const double* qin, double* qout, const 
     } else {
         const int seg = pick_seg(P.ny, 1, 128);
         dim3 grid((P.nx + YT - 1) / YT, (P.ny + seg - 1) / seg);
-        if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, YT, 0, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, YT, 0, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_ysweep<MODE_TRAIL><<<grid, YT, 0, s>>>(P, qin, qout, dtp, ctl, seg);
+        const size_t sm = YS_DOUBLES * sizeof(double);
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaFuncSetAttribute(k_ysweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            cudaFuncSetAttribute(k_ysweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            cudaFuncSetAttribute(k_ysweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            attr_done = true;
+        }
+        if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_ysweep<MODE_TRAIL><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
     }
 }
 
