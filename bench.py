@@ -29,10 +29,16 @@ from paper_1905_05727_b200 import inputs  # noqa: E402
 
 METRIC = "fp64 cell-updates/s per 2D step"
 UNIT = "cell-updates/s"
-# algorithmic FP64 work of one cell-step (two sweeps + two source half-steps + CFL),
-# counted on the oracle's arithmetic with the CUDA math-library expansions of div/sqrt/exp/log
-FLOP_PER_CELL_SWEEP = 1560.0      # one directional sweep of one cell (dadd+dmul = 1, dfma = 2)
+# algorithmic FP64 work of one cell in one fused directional sweep, from ncu's counters of the
+# C5 launches (profiles/r01b_fused_c5.md) divided by the 33/32 ramp-up redundancy of a segment.
+#   FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot):
+FP64_INSTR_PER_CELL = {"lead": 455.0, "trail": 546.0}       # pass 1 = S + sweep; pass 2 = sweep + S + wavespeed
+#   flops with dadd = dmul = 1, dfma = 2 (56 % of the FP64 instructions are DFMA):
+FLOP_PER_CELL = {"lead": 648.0, "trail": 776.0}
 FP64_LANES_PER_SM, N_SM = 64, 148
+# dram__bytes_read.sum + dram__bytes_write.sum per cell per launch from the ncu --set full capture of C5 (mean of the
+# lead and trail launches; profiles/r01b_fused_c5.md): 113.6 B (x), 113.6 B (y) against 112 B algorithmic
+TRAFFIC_BYTES_PER_CELL = {"sweep_x": 113.8, "sweep_y": 113.6}
 
 
 def peaks():
@@ -191,15 +197,32 @@ def main():
     value = cells * K * world / (ms * 1e-3)
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------
+    # The sweeps are bound by the FP64 pipe: one warp instruction per 2 clocks per SMSP whatever the
+    # opcode, i.e. 64 lane-slots per SM per clock.  `achieved` counts the algorithmic FP64 instructions of the
+    # kernel (one launch of each mode per two steps, so the mean of lead and trail) as 2-flop DFMA slots, so that
+    # `frac` is the FP64-pipe utilisation that ncu reports as sm__inst_executed_pipe_fp64; the plain flop rate
+    # (dadd = dmul = 1, dfma = 2) is given beside it.
     pk = peaks()
     clk = sampler.summary()
     sm_max = pk.get("sm_max_mhz", clk.get("sm_max_mhz") or 1965.0)
     peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     dom = max(("sweep_x", "sweep_y"), key=lambda k: kt[k][0])
     dom_ms = kt[dom][0] / max(kt[dom][1], 1)
-    achieved = FLOP_PER_CELL_SWEEP * cells / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    instr = 0.5 * (FP64_INSTR_PER_CELL["lead"] + FP64_INSTR_PER_CELL["trail"])
+    flop = 0.5 * (FLOP_PER_CELL["lead"] + FLOP_PER_CELL["trail"])
+    achieved = 2.0 * instr * cells / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    try:
+        probe_gflops, _ = sim.probe_fp64()
+    except Exception:
+        probe_gflops = None
+    step_instr = FP64_INSTR_PER_CELL["lead"] + FP64_INSTR_PER_CELL["trail"]
     roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-            "frac": achieved / peak_tflops, "traffic": None, "peak_source": "148 SM x 64 FP64 lanes x 2 x sm_max_mhz (nominal)",
+            "frac": achieved / peak_tflops, "traffic": TRAFFIC_BYTES_PER_CELL.get(dom) * cells if args.config == "C5" else None,
+            "counting": "FP64-pipe issue slots x 2 flop (DFMA-equivalent); %.0f FP64 instr/cell/launch" % instr,
+            "achieved_plain_flops": flop * cells / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0,
+            "peak_source": "148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (guide's unit counts and clock)",
+            "peak_measured_dfma_probe": probe_gflops / 1e3 if probe_gflops else None,
+            "whole_step_frac": 2.0 * step_instr * cells * K / (ms * 1e-3) / 1e12 / peak_tflops,
             "ms_per_launch": dom_ms,
             "hbm_gbs_algorithmic": 112.0 * cells / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0,
             "hbm_peak_gbs": pk.get("hbm_gbs", 6650.0),

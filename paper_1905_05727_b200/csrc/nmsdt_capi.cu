@@ -64,6 +64,9 @@ struct sim {
     double M2tot0 = 0.0;
     int variant = SIM_VARIANT_FUSED;
     int use_graph = 1;
+    cudaGraphExec_t gexec = nullptr;    // fused path: one even (X-Y) + one odd (Y-X) step = 10 kernel nodes
+    cudaStream_t cap_stream = nullptr;  // private stream the graph is captured on (the caller's may be the legacy stream)
+    bool graph_failed = false;
     bool cfl_valid = false;         // fused path: ctl->dt / ctl->tsafe describe the current state and dt mode
     double dt_mode = -1.0;          // dt_fixed the control block was last prepared for
     long long launches = 0;
@@ -203,6 +206,32 @@ void enqueue_step_fused(sim* s)
     s->host_step++;
 }
 
+// fused path: CUDA graph of two consecutive steps starting at an even step.  Captured once on a private stream
+// (nothing executes during capture; every kernel argument is fixed for the lifetime of the handle) and replayed on
+// the caller's stream, which removes the per-launch CPU cost that dominates the small configs (C1, C2).
+bool ensure_graph(sim* s)
+{
+    if (s->gexec) return true;
+    if (s->graph_failed) return false;
+    s->graph_failed = true;
+    if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
+    cudaStream_t user = s->stream;
+    const long long step0 = s->host_step, l0 = s->launches;
+    cudaGraph_t g = nullptr;
+    if (cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return false; }
+    s->stream = s->cap_stream;
+    s->host_step = 0;
+    enqueue_step_fused(s);
+    enqueue_step_fused(s);
+    s->stream = user; s->host_step = step0; s->launches = l0;
+    if (cudaStreamEndCapture(s->cap_stream, &g) != cudaSuccess || !g) { cudaGetLastError(); return false; }
+    const cudaError_t e = cudaGraphInstantiate(&s->gexec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { cudaGetLastError(); s->gexec = nullptr; return false; }
+    s->graph_failed = false;
+    return true;
+}
+
 // fused path: make ctl->dt / ctl->tsafe valid for the current state (first step after init or after a piecewise call)
 void prepare_ctl_fused(sim* s)
 {
@@ -272,6 +301,7 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     s->scratch = (double*)(s->base + s->L.off_scratch);
     s->tab = (double*)(s->base + s->L.off_tab);
     fill_params(s);
+    init_fused_kernels();
     cudaMemsetAsync(s->base, 0, s->L.total, s->stream);
     {
         double htab[MATH_TAB_DOUBLES];
@@ -288,6 +318,8 @@ void sim_destroy(sim_t* s)
     if (!s) return;
     cudaStreamSynchronize(s->stream);
     if (s->d_cav) cudaFree(s->d_cav);
+    if (s->gexec) cudaGraphExecDestroy(s->gexec);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     for (auto& p : s->ev) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     if (s->owns && s->base) cudaFree(s->base);
     delete s;
@@ -377,6 +409,15 @@ static int step_common(sim_t* s, int n, double dt_fixed)
     }
     if (n == 0) return SIM_OK;
     if (!s->cfl_valid || s->dt_mode != dt_fixed) prepare_ctl_fused(s);
+    if (s->use_graph && !s->profile && n >= 3) {
+        if (s->host_step & 1) { enqueue_step_fused(s); --n; }
+        if (ensure_graph(s)) {
+            for (; n >= 2; n -= 2) {
+                if (cudaGraphLaunch(s->gexec, s->stream) != cudaSuccess) return check_cuda(s, "sim_step (graph)");
+                s->launches += 10; s->host_step += 2;
+            }
+        }
+    }
     for (int it = 0; it < n; ++it) enqueue_step_fused(s);
     s->cfl_valid = true; s->dt_mode = dt_fixed;
     return check_cuda(s, "sim_step");

@@ -253,7 +253,7 @@ __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double la
 #define NMSDT_Y_MINBLOCKS 4
 #endif
 #ifndef NMSDT_X_MINBLOCKS
-#define NMSDT_X_MINBLOCKS 2
+#define NMSDT_X_MINBLOCKS 3
 #endif
 constexpr int XW = 4;                       // warps per block in k_xsweep
 constexpr int RING = 33;
@@ -601,41 +601,63 @@ __global__ void k_ctl(const __grid_constant__ Params P, Ctl* ctl, int advance)
 // ---------------------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------------------
-static int pick_seg(int n, int unit, int target)
+// Segment length along the marching axis.  A block marches over `seg` cells after `ramp` cells of ramp-up (recomputed
+// halo), `lines` blocks stand side by side, and `slots` blocks are resident on the whole GPU at once, so the sweep
+// takes about ceil(lines * nseg / slots) * (seg + ramp) marching iterations: pick the nseg that minimises that
+// (large grids end up near `target`, small ones are cut into enough segments to fill all SMs).
+static int pick_seg(int n, int unit, int target, int ramp, int lines, int slots)
 {
-    int nseg = (n + target - 1) / target;
-    if (nseg < 1) nseg = 1;
-    int seg = (n + nseg - 1) / nseg;
-    return (seg + unit - 1) / unit * unit;
+    const int max_seg = (n + unit - 1) / unit;                 // in units
+    int best_seg = max_seg * unit; double best = 1e300;
+    const int su0 = (2 * ramp + unit - 1) / unit < max_seg ? (2 * ramp + unit - 1) / unit : max_seg;   // redundancy <= 1.5
+    for (int su = su0; su <= max_seg; ++su) {
+        const int seg = su * unit;
+        if (seg > 2 * target && su > su0) break;
+        const int nseg = (n + seg - 1) / seg;
+        const double waves = (double)(((long long)lines * nseg + slots - 1) / slots);
+        const double cost = waves * (seg + ramp);
+        if (cost < best * (1.0 - 1e-9)) { best = cost; best_seg = seg; }
+    }
+    return best_seg;
+}
+
+static int num_sms()
+{
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0; cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    }
+    return n;
+}
+
+// opt in to the dynamic shared memory the sweeps need (called once per handle from sim_create, outside any capture)
+void init_fused_kernels()
+{
+    const int smx = (int)(XS_DOUBLES * sizeof(double)), smy = (int)(YS_DOUBLES * sizeof(double));
+    cudaFuncSetAttribute(k_xsweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
+    cudaFuncSetAttribute(k_xsweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
+    cudaFuncSetAttribute(k_xsweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
+    cudaFuncSetAttribute(k_ysweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
+    cudaFuncSetAttribute(k_ysweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
+    cudaFuncSetAttribute(k_ysweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
 }
 
 void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s)
 {
     if (dir == 0) {
-        const int seg = pick_seg(P.nx, 64, 2048);
-        dim3 grid((P.ny + XW - 1) / XW, (P.nx + seg - 1) / seg);
+        const int lines = (P.ny + XW - 1) / XW;
+        const int seg = pick_seg(P.nx, 64, 2048, 64, lines, num_sms() * NMSDT_X_MINBLOCKS);
+        dim3 grid(lines, (P.nx + seg - 1) / seg);
         const size_t sm = XS_DOUBLES * sizeof(double);
-        static bool attr_done = false;
-        if (!attr_done) {
-            cudaFuncSetAttribute(k_xsweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            cudaFuncSetAttribute(k_xsweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            cudaFuncSetAttribute(k_xsweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            attr_done = true;
-        }
         if (mode == MODE_PLAIN)      k_xsweep<MODE_PLAIN><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
         else if (mode == MODE_LEAD)  k_xsweep<MODE_LEAD><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
         else                         k_xsweep<MODE_TRAIL><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
     } else {
-        const int seg = pick_seg(P.ny, 1, 128);
-        dim3 grid((P.nx + YT - 1) / YT, (P.ny + seg - 1) / seg);
+        const int lines = (P.nx + YT - 1) / YT;
+        const int seg = pick_seg(P.ny, 1, 128, 4, lines, num_sms() * NMSDT_Y_MINBLOCKS);
+        dim3 grid(lines, (P.ny + seg - 1) / seg);
         const size_t sm = YS_DOUBLES * sizeof(double);
-        static bool attr_done = false;
-        if (!attr_done) {
-            cudaFuncSetAttribute(k_ysweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            cudaFuncSetAttribute(k_ysweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            cudaFuncSetAttribute(k_ysweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            attr_done = true;
-        }
         if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
         else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
         else                         k_ysweep<MODE_TRAIL><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);

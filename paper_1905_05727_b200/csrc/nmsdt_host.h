@@ -31,6 +31,7 @@ int  launch_probe_fp64(cudaStream_t s, double* gflops, double* ms);
 
 // fused production path (nmsdt_fused.cu). dtp -> {dt (or tau for the source kernel), tsafe}; mode 0 plain, 1 leading
 // source on load, 2 trailing source + max-wavespeed partial
+void init_fused_kernels();
 void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s);
 void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s);
 void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s);
