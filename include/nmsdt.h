@@ -147,6 +147,14 @@ int sim_profile(sim_t*, int on);
 int sim_kernel_time(const sim_t*, int kind, double* ms_total, long long* launches);
 /* Measured FP64 FMA throughput of this device in GFLOP/s (2 flop per DFMA), probe kernel of ~ms. [sync] */
 int sim_probe_fp64(sim_t*, double* gflops_out, double* ms_out);
+/* Accuracy probe of the fused path's own fp64 elementary functions (the Cochran-Chan powers of Eq. 3-4, and
+   the Arrhenius exponential of Eq. 6, are evaluated with these instead of the CUDA math library; DESIGN.md
+   section 5).  Evaluates function `fn` on host_x[n] on the device and returns host_y0[n], host_y1[n] (HOST arrays,
+   caller-owned; y1 is written with zeros when the function has one result):
+     0: 1/x            1: sqrt(x)        2: ln(x)        3: (x^a, x^b)        4: exp(-x)
+     5: (max(x,1), min(max(x,0),1))      6: (max(x,0), min(x,690))
+   x must be a positive normal number for 0-3. SIM_ERR_ARG on NULL / n < 1 / unknown fn. [sync] */
+int sim_probe_math(sim_t*, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1);
 
 #ifdef __cplusplus
 }

@@ -22,7 +22,7 @@ FIELD = {"q0": 0, "q1": 1, "q2": 2, "q3": 3, "q4": 4, "q5": 5, "q6": 6, "p": 16,
 SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error", "sim_init", "sim_init_fields",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
            "sim_read_field", "sim_get_cavities", "sim_set_variant", "sim_launch_count", "sim_device_layout",
-           "sim_probe_fp64", "sim_profile", "sim_kernel_time"]
+           "sim_probe_fp64", "sim_probe_math", "sim_profile", "sim_kernel_time"]
 KERNEL_KINDS = {"sweep_x": 0, "sweep_y": 1, "source": 2, "cfl": 3, "halo": 4}
 
 
@@ -101,6 +101,7 @@ def load_library():
         "sim_device_layout": (C.c_int, [vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(C.c_int),
                                         C.POINTER(C.c_int), C.POINTER(C.c_int)]),
         "sim_probe_fp64": (C.c_int, [vp, dp, dp]),
+        "sim_probe_math": (C.c_int, [vp, C.c_int, dp, C.c_int, C.c_double, C.c_double, dp, dp]),
         "sim_profile": (C.c_int, [vp, C.c_int]),
         "sim_kernel_time": (C.c_int, [vp, C.c_int, dp, C.POINTER(C.c_longlong)]),
     }
@@ -242,6 +243,15 @@ class Sim:
         g, ms = C.c_double(), C.c_double()
         self._chk(self.L.sim_probe_fp64(self.h, C.byref(g), C.byref(ms)), "sim_probe_fp64")
         return g.value, ms.value
+
+    def probe_math(self, fn, x, a=0.0, b=0.0):
+        """device evaluation of the fused path's elementary functions (include/nmsdt.h: sim_probe_math)"""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y0, y1 = np.empty_like(x), np.empty_like(x)
+        dp = C.POINTER(C.c_double)
+        self._chk(self.L.sim_probe_math(self.h, int(fn), x.ctypes.data_as(dp), int(x.size), float(a), float(b),
+                                        y0.ctypes.data_as(dp), y1.ctypes.data_as(dp)), "sim_probe_math")
+        return y0, y1
 
     def profile(self, on):
         self._chk(self.L.sim_profile(self.h, int(bool(on))), "sim_profile")

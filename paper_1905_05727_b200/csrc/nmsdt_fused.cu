@@ -57,13 +57,13 @@ __device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* _
     double lam = lam0;
     for (int s = 0; s < nsub; ++s) {
         double l, T, k1, k2, k3, k4;
-        l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = T > 0.0 ? k1 : 0.0;
-        l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = T > 0.0 ? k2 : 0.0;
-        l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = T > 0.0 ? k3 : 0.0;
-        l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = T > 0.0 ? k4 : 0.0;
+        l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = is_pos(T) ? k1 : 0.0;
+        l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = is_pos(T) ? k2 : 0.0;
+        l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = is_pos(T) ? k3 : 0.0;
+        l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = is_pos(T) ? k4 : 0.0;
         lam = fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
     }
-    return clampf(lam, 0.0, lam0);
+    return dmin_(nonneg(lam), lam0);
 }
 
 // O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.
@@ -92,7 +92,7 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double ixi = q_rcp(xi);
     double p = (rhoe - z2 * fma(-pr, P.iG2, rer)) * ixi;
-    double lam = clampf(q[6] * iq1, 0.0, 1.0);
+    double lam = clamp01(q[6] * iq1);
     dE = 0.0; q6n = q[6];
     if (SRC) {
         if (P.reactive) {
@@ -127,7 +127,7 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
     const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22);
-    f.c = q_sqrt(dmax_(rc2 * q_rcp(xi * rho), 1.0));
+    f.c = q_sqrt(floor1(rc2 * q_rcp(xi * rho)));
 }
 
 __device__ __forceinline__ double limited_f(int kind, double a, double b)
@@ -142,16 +142,14 @@ __device__ __forceinline__ double limited_f(int kind, double a, double b)
     return a * b > 0.0 ? m : 0.0;
 }
 
-// O4.1-2 for the centre cell W0
-__device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, const FCell& W0, const FCell& Wp, double khalf, double WL[7],
+// O4.1-2 for the centre cell W0, given the one-sided differences a = W0 - W(-1), b = W(+1) - W0
+__device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, const double a[7], const double b[7], double khalf, double WL[7],
                                            double WR[7])
 {
     const double w0[7] = {W0.r1, W0.r2, W0.un, W0.ut, W0.p, W0.z1, W0.lam};
-    const double wm[7] = {Wm.r1, Wm.r2, Wm.un, Wm.ut, Wm.p, Wm.z1, Wm.lam};
-    const double wp[7] = {Wp.r1, Wp.r2, Wp.un, Wp.ut, Wp.p, Wp.z1, Wp.lam};
     double D[7];
 #pragma unroll
-    for (int k = 0; k < 7; ++k) D[k] = limited_f(P.limiter, w0[k] - wm[k], wp[k] - w0[k]);
+    for (int k = 0; k < 7; ++k) D[k] = limited_f(P.limiter, a[k], b[k]);
     const double u = W0.un;
     double d[7];
     d[0] = fma(u, D[0], W0.r1 * D[2]);
@@ -167,11 +165,21 @@ __device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, con
         WL[k] = fma(-0.5, D[k], m);
         WR[k] = fma(0.5, D[k], m);
     }
-    const bool ok = (WL[0] > 0.0) && (WL[1] > 0.0) && (WR[0] > 0.0) && (WR[1] > 0.0);     // R17
-    if (!ok) {
+    // R17 first-order fallback.  It practically never fires, so it sits behind a warp-uniform branch instead of 14
+    // unconditional selects.
+    const bool ok = min(min(hi_word(WL[0]), hi_word(WL[1])), min(hi_word(WR[0]), hi_word(WR[1]))) > 0;   // all four > 0
+    if (__any_sync(__activemask(), !ok)) {
 #pragma unroll
-        for (int k = 0; k < 7; ++k) { WL[k] = w0[k]; WR[k] = w0[k]; }
+        for (int k = 0; k < 7; ++k) { WL[k] = ok ? WL[k] : w0[k]; WR[k] = ok ? WR[k] : w0[k]; }
     }
+}
+
+__device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, const FCell& W0, const FCell& Wp, double khalf, double WL[7],
+                                           double WR[7])
+{
+    const double a[7] = {W0.r1 - Wm.r1, W0.r2 - Wm.r2, W0.un - Wm.un, W0.ut - Wm.ut, W0.p - Wm.p, W0.z1 - Wm.z1, W0.lam - Wm.lam};
+    const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
+    recon_core(P, W0, a, b, khalf, WL, WR);
 }
 
 // O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
@@ -259,7 +267,7 @@ constexpr int XW = 4;                       // warps per block in k_xsweep
 constexpr int RING = 33;
 constexpr int RING_DOUBLES = (16 + 10 + 8) * RING;
 constexpr int PRING = 66;                   // staged input pairs: chunk k (32 slots), chunk k+1 in flight, lane 31 of chunk k-1
-constexpr int XS_DOUBLES = MATH_TAB_DOUBLES + XW * (RING_DOUBLES + 7 * PRING * 2);
+constexpr int XS_DOUBLES = XW * (RING_DOUBLES + 7 * PRING * 2);    // dynamic part (the math tables are static)
 
 } // namespace
 
@@ -282,7 +290,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 constexpr int YT = 128;      // threads (columns) per block in k_ysweep
 constexpr int YST = 3;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1 in flight
-constexpr int YS_DOUBLES = MATH_TAB_DOUBLES + (YST * 7 + 2 * 9 + 10) * YT;
+constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part (the math tables are static)
 
 // Per-thread state that lives across rows is kept in thread-private shared-memory slots ([..][YT] layout, conflict
 // free, no barriers): the staged input rows, the primitive window (cells c-2, c-1) and the previous right-face state.
@@ -292,10 +300,10 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
                                                                   double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
     extern __shared__ __align__(16) double s_dyn[];
-    double* s_tab = s_dyn;
-    double (*s_q)[7][YT] = reinterpret_cast<double (*)[7][YT]>(s_dyn + MATH_TAB_DOUBLES);
-    double (*s_w)[9][YT] = reinterpret_cast<double (*)[9][YT]>(s_dyn + MATH_TAB_DOUBLES + YST * 7 * YT);
-    double (*s_r)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + MATH_TAB_DOUBLES + (YST * 7 + 2 * 9) * YT);
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];     // static: table lookups address it as [idx + const]
+    double (*s_q)[7][YT] = reinterpret_cast<double (*)[7][YT]>(s_dyn);
+    double (*s_w)[9][YT] = reinterpret_cast<double (*)[9][YT]>(s_dyn + YST * 7 * YT);
+    double (*s_r)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + (YST * 7 + 9 + 7) * YT);
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int tid = threadIdx.x;
@@ -337,19 +345,22 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
             }
             // The body is branch free: during the 4 ramp-up rows it runs on not-yet-valid window / face / flux values
             // (finite or not, never stored: the store and the wavespeed contribution are predicated on jj >= 4).
-            const int wm = jj & 1, w0 = wm ^ 1;       // window slots of cells c-2 and c-1
             double WL[7], WR[7], lam0c;
-            {                                         // centre cell c-1
-                FCell Wm, W0;
-                Wm.r1 = s_w[wm][0][tid]; Wm.r2 = s_w[wm][1][tid]; Wm.un = s_w[wm][2][tid]; Wm.ut = s_w[wm][3][tid]; Wm.p = s_w[wm][4][tid];
-                Wm.z1 = s_w[wm][5][tid]; Wm.lam = s_w[wm][6][tid]; Wm.irho = 0.0; Wm.rc2 = 0.0;
-                W0.r1 = s_w[w0][0][tid]; W0.r2 = s_w[w0][1][tid]; W0.un = s_w[w0][2][tid]; W0.ut = s_w[w0][3][tid]; W0.p = s_w[w0][4][tid];
-                W0.z1 = s_w[w0][5][tid]; W0.lam = s_w[w0][6][tid]; W0.irho = s_w[w0][7][tid]; W0.rc2 = s_w[w0][8][tid];
+            {                                         // centre cell c-1: s_w[0] = W(c-1), s_w[1][0..6] = W(c-1) - W(c-2)
+                FCell W0;
+                W0.r1 = s_w[0][0][tid]; W0.r2 = s_w[0][1][tid]; W0.un = s_w[0][2][tid]; W0.ut = s_w[0][3][tid]; W0.p = s_w[0][4][tid];
+                W0.z1 = s_w[0][5][tid]; W0.lam = s_w[0][6][tid]; W0.irho = s_w[0][7][tid]; W0.rc2 = s_w[0][8][tid];
+                double a[7];
+#pragma unroll
+                for (int k = 0; k < 7; ++k) a[k] = s_w[1][k][tid];
+                const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
                 lam0c = W0.lam;
-                recon_fast(P, Wm, W0, Wp, khalf, WL, WR);
+                recon_core(P, W0, a, b, khalf, WL, WR);
+#pragma unroll
+                for (int k = 0; k < 7; ++k) s_w[1][k][tid] = b[k];
             }
-            s_w[wm][0][tid] = Wp.r1; s_w[wm][1][tid] = Wp.r2; s_w[wm][2][tid] = Wp.un; s_w[wm][3][tid] = Wp.ut; s_w[wm][4][tid] = Wp.p;
-            s_w[wm][5][tid] = Wp.z1; s_w[wm][6][tid] = Wp.lam; s_w[wm][7][tid] = Wp.irho; s_w[wm][8][tid] = Wp.rc2;
+            s_w[0][0][tid] = Wp.r1; s_w[0][1][tid] = Wp.r2; s_w[0][2][tid] = Wp.un; s_w[0][3][tid] = Wp.ut; s_w[0][4][tid] = Wp.p;
+            s_w[0][5][tid] = Wp.z1; s_w[0][6][tid] = Wp.lam; s_w[0][7][tid] = Wp.irho; s_w[0][8][tid] = Wp.rc2;
             FFace fl, fr, pr;
             face_fast(P, s_tab, WL, fl);
             face_fast(P, s_tab, WR, fr);
@@ -403,8 +414,8 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
                                                     const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
     extern __shared__ __align__(16) double s_dyn[];
-    double* s_tab = s_dyn;
-    double* s_ring = s_dyn + MATH_TAB_DOUBLES;
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
+    double* s_ring = s_dyn;
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -414,7 +425,7 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
         double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
         double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
         double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
-        double2* stg = reinterpret_cast<double2*>(s_dyn + MATH_TAB_DOUBLES + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
+        double2* stg = reinterpret_cast<double2*>(s_dyn + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
         const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
         const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
         const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
@@ -673,5 +684,46 @@ void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStrea
 void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s) { k_ctl<<<1, 1, 0, s>>>(P, ctl, advance); }
 
 double host_tsafe(double tau, double Cpre, double Ta, double theta0) { return tsafe_for(tau, Cpre, Ta, theta0); }
+
+// ---------------------------------------------------------------------------------------------------------------
+// sim_probe_math: evaluate the elementary functions of nmsdt_math.cuh on device arrays (accuracy tests)
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_probe_math(const double* __restrict__ tab_g, int fn, const double* __restrict__ x, int n, double a, double b,
+                                                    double* __restrict__ y0, double* __restrict__ y1)
+{
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
+    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = tab_g[i];
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v = x[i];
+    double r0 = 0.0, r1 = 0.0;
+    switch (fn) {
+    case 0: r0 = q_rcp(v); break;
+    case 1: r0 = q_sqrt(v); break;
+    case 2: r0 = q_log(s_tab, v); break;
+    case 3: q_pow_pair(s_tab, v, a * LOG2E, b * LOG2E, r0, r1); break;      // (v^a, v^b)
+    case 4: r0 = q_exp_neg(s_tab, v); break;
+    case 5: r0 = floor1(v); r1 = clamp01(v); break;
+    case 6: r0 = nonneg(v); r1 = cap690(v); break;
+    default: break;
+    }
+    y0[i] = r0; y1[i] = r1;
+}
+
+int launch_probe_math(const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
+                      cudaStream_t s)
+{
+    double *dx = nullptr, *dy = nullptr;
+    if (cudaMalloc(&dx, sizeof(double) * n) != cudaSuccess) return -2;
+    if (cudaMalloc(&dy, sizeof(double) * 2 * n) != cudaSuccess) { cudaFree(dx); return -2; }
+    cudaMemcpyAsync(dx, host_x, sizeof(double) * n, cudaMemcpyHostToDevice, s);
+    k_probe_math<<<(n + 127) / 128, 128, 0, s>>>(tab_dev, fn, dx, n, a, b, dy, dy + n);
+    cudaMemcpyAsync(host_y0, dy, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(host_y1, dy + n, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
+    const cudaError_t e = cudaStreamSynchronize(s);
+    cudaFree(dx); cudaFree(dy);
+    return e == cudaSuccess ? 0 : -2;
+}
 
 } // namespace nmsdt

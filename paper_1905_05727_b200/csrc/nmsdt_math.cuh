@@ -6,12 +6,14 @@
 // special-case handling is dropped and the functions are rebuilt from the MUFU seeds (rcp.approx / rsqrt.approx,
 // ~20 bits) + Newton steps and from two small tables held in shared memory:
 //   q_rcp   1 MUFU + 3 DFMA          (<= 1 ulp for normal x)
-//   q_sqrt  1 MUFU + 2 DMUL + 5 DFMA   (~1 ulp)
-//   pow_pair(x) -> (x^C, x^D)  Eq. 3-4: one table-driven log (128 entries, degree-6 log1p) and two
-//          table-driven exp2 (64 entries, degree-5), 28 FP64 instructions instead of ~90
+//   q_sqrt  1 MUFU + 2 DMUL + 3 DFMA   (~1 ulp)
+//   pow_pair(x) -> (x^C, x^D)  Eq. 3-4: one table-driven log (256 entries, degree-5 log1p) and two
+//          table-driven exp2 (256 entries, degree-4), 25 FP64 instructions instead of ~90
 //   exp_neg(y) = e^-y for the Arrhenius factor of Eq. 6
-// Accuracy (checked on the device by tests/test_gpu_math.py against long-double references): relative error
-// <= 4e-16 for q_rcp/q_sqrt, <= 2e-15 for the powers over rho2/rho02 in [1e-3, 1e3].
+// Accuracy (tests/math_cases.py: on the host by tests/test_math_host.py, on the device by tests/test_gpu_math.py through
+// sim_probe_math, against long-double library references): relative error <= 2e-16 for q_rcp / q_sqrt, absolute
+// error <= 2e-16 max(1, |ln x|) for q_log, <= 8e-16 + 3e-16 |a ln x| for the powers x^a (1.2e-15 for rho2/rho02 in
+// [0.5, 3]), <= 1e-15 for exp(-y), y <= 40.
 // Compiles for the host too (HOST_SEED emulates the 20-bit seeds) so that the polynomial/table logic can be checked
 // without a GPU.  Shares nothing with oracle/.
 #pragma once
@@ -21,9 +23,9 @@
 
 namespace nmsdt {
 
-constexpr int LOG_TAB_BITS = 7, LOG_TAB_N = 1 << LOG_TAB_BITS;     // (1/c_j, ln c_j) pairs
-constexpr int EXP_TAB_BITS = 6, EXP_TAB_N = 1 << EXP_TAB_BITS;     // 2^(j/64)
-constexpr int MATH_TAB_DOUBLES = 2 * LOG_TAB_N + EXP_TAB_N;        // 320 doubles = 2560 B of shared memory
+constexpr int LOG_TAB_BITS = 8, LOG_TAB_N = 1 << LOG_TAB_BITS;     // (1/c_j, ln c_j) pairs
+constexpr int EXP_TAB_BITS = 8, EXP_TAB_N = 1 << EXP_TAB_BITS;     // 2^(j/256)
+constexpr int MATH_TAB_DOUBLES = 2 * LOG_TAB_N + EXP_TAB_N;        // 768 doubles = 6144 B of shared memory
 
 #if defined(__CUDA_ARCH__)
 #define NMSDT_HD __device__ __forceinline__
@@ -49,8 +51,8 @@ inline double rsq_seed(double x) { return mk_double(hi_word(1.0 / sqrt(mk_double
 #define NMSDT_KCONST static const double
 #endif
 NMSDT_KCONST KC[10] = {
-    -1.0 / 6.0, 0.2, 1.0 / 3.0, 0.69314718055994530942,                                  // log1p series, ln 2
-    1.3333558146428443e-3, 9.6181291076284772e-3, 5.5504108664821580e-2,                 // ln2^5/120, ln2^4/24, ln2^3/6
+    0.0, 0.2, 1.0 / 3.0, 0.69314718055994530942,                                         // (unused), log1p series, ln 2
+    0.0, 9.6181291076284772e-3, 5.5504108664821580e-2,                                   // (unused), ln2^4/24, ln2^3/6
     2.4022650695910071e-1, 6.9314718055994531e-1, 1.4426950408889634074};                // ln2^2/2, ln2, log2(e)
 
 // min / max without the NaN rules of fmin / fmax (3 instructions instead of 5-6; operands here are never NaN on a
@@ -67,16 +69,28 @@ NMSDT_HD double q_rcp(double x)
     return fma(r, e, r);
 }
 
-// sqrt(x) for positive normal x (coupled Newton iteration on sqrt and 1/(2 sqrt))
+// sqrt(x) for positive normal x: seed y ~ (1+d)/sqrt(x), e = 1 - x y^2, sqrt(x) = x y (1-e)^(-1/2) truncated after the
+// e^2 term (next term 5/16 e^3 < 3e-18 for the 2^-20 seed): 2 DMUL + 3 DFMA
 NMSDT_HD double q_sqrt(double x)
 {
-    double y = rsq_seed(x);
-    double g = x * y, h = 0.5 * y;
-    double e = fma(-g, h, 0.5);
-    g = fma(g, e, g); h = fma(h, e, h);
-    e = fma(-g, h, 0.5);
-    return fma(g, e, g);
+    const double y = rsq_seed(x);
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(e, 0.375, 0.5) * e;
+    return fma(t, p, t);
 }
+
+// Clamps decided on the high word (integer pipe instead of the FP64 pipe).  For finite x:
+//   floor1(x)  = max(x, 1)      (x < 1, zero or negative -> 1; the signed compare sends negative x below 0x3ff00000)
+//   clamp01(x) = min(max(x, 0), 1)
+//   nonneg(x)  = max(x, 0)
+//   cap690(y)  = min(y, 690) for the argument of exp(-y) (690 = 0x40859000_00000000 exactly)
+//   is_pos(x)  = x > 0 for x that is zero, normal or infinite (a positive subnormal counts as zero)
+NMSDT_HD bool is_pos(double x) { return hi_word(x) > 0; }
+NMSDT_HD double floor1(double x) { return hi_word(x) >= 0x3ff00000 ? x : 1.0; }
+NMSDT_HD double nonneg(double x) { return hi_word(x) < 0 ? 0.0 : x; }
+NMSDT_HD double clamp01(double x) { const int h = hi_word(x); return h < 0 ? 0.0 : (h >= 0x3ff00000 ? 1.0 : x); }
+NMSDT_HD double cap690(double y) { return hi_word(y) < 0x40859000 ? y : 690.0; }
 
 // ln(x), x positive normal.  tab = shared-memory copy of the tables.  Absolute error ~1e-16 (+ 1 ulp of the result).
 NMSDT_HD double q_log(const double* __restrict__ tab, double x)
@@ -86,9 +100,8 @@ NMSDT_HD double q_log(const double* __restrict__ tab, double x)
     const double m = mk_double((hx & 0x000fffff) | 0x3ff00000, lo_word(x));            // mantissa in [1,2)
     const double ed = mk_double(0x43300000, hx >> 20) - 4503599627371519.0;             // unbiased exponent: (2^52 + e_biased) - (2^52 + 1023)
     const double ic = tab[2 * j], lc = tab[2 * j + 1];
-    const double r = fma(m, ic, -1.0);                                                 // |r| <= 2^-8
-    double p = fma(r, KC[0], KC[1]);
-    p = fma(p, r, -0.25);
+    const double r = fma(m, ic, -1.0);                                                 // |r| <= 2^-9: r^6/6 < 1e-17
+    double p = fma(r, KC[1], -0.25);
     p = fma(p, r, KC[2]);
     p = fma(p, r, -0.5);
     p = fma(p, r * r, r);                                                              // log1p(r)
@@ -98,13 +111,12 @@ NMSDT_HD double q_log(const double* __restrict__ tab, double x)
 // 2^(a*b) for |a*b| < 1000 (a*b is never rounded: the reduction uses the exact product through fma)
 NMSDT_HD double q_exp2_prod(const double* __restrict__ tab, double a, double b)
 {
-    const double SH = 6755399441055744.0 / EXP_TAB_N;           // 1.5 * 2^52 / 64: ulp = 1/64
+    const double SH = 6755399441055744.0 / EXP_TAB_N;           // 1.5 * 2^52 / 256: ulp = 1/256
     const double t = fma(a, b, SH);
     const int N = lo_word(t);
-    const double f = fma(a, b, -(t - SH));                      // |f| <= 1/128
+    const double f = fma(a, b, -(t - SH));                      // |f| <= 1/512: (f ln2)^5/120 < 4e-17
     const double T = tab[2 * LOG_TAB_N + (N & (EXP_TAB_N - 1))];
-    double p = fma(f, KC[4], KC[5]);
-    p = fma(p, f, KC[6]);
+    double p = fma(f, KC[5], KC[6]);
     p = fma(p, f, KC[7]);
     p = fma(p, f, KC[8]);
     const double v = fma(T, p * f, T);
@@ -124,7 +136,7 @@ NMSDT_HD void q_pow_pair(const double* __restrict__ tab, double x, double C2, do
 // e^(-y) for y >= 0 (flushes to ~1e-301 for y > 690)
 NMSDT_HD double q_exp_neg(const double* __restrict__ tab, double y)
 {
-    return q_exp2_prod(tab, dmin_(y, 690.0), -KC[9]);
+    return q_exp2_prod(tab, cap690(y), -KC[9]);
 }
 
 // host side: fill the 320-double table (long double arithmetic)
