@@ -45,23 +45,39 @@ __device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
     return (r >= (double)(P.max_substeps - 1)) ? P.max_substeps : 1 + (int)r;
 }
 
-// O5: lambda after integrating d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)) over tau, T2 = T0 + beta (lam0 - lambda)
+// one classic RK4 step of d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)), T2 = T0 + beta (lam0 - lambda), from lam over h
+__device__ __forceinline__ double rk4_step(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double lam,
+                                           double h)
+{
+    const double nTa = P.Ta, mC = -P.Cpre;
+    double l, T, k1, k2, k3, k4;
+    l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = is_pos(T) ? k1 : 0.0;
+    l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = is_pos(T) ? k2 : 0.0;
+    l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = is_pos(T) ? k3 : 0.0;
+    l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = is_pos(T) ? k4 : 0.0;
+    return fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
+}
+
+// R13 sub-stepped integration (only reached by cells hotter than the safe bound)
+__device__ __noinline__ double rk4_substepped(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double tau)
+{
+    const int nsub = nsub_exact(P, fma(beta, lam0, T0), tau);
+    const double h = tau / (double)nsub;
+    double lam = lam0;
+    for (int s = 0; s < nsub; ++s) lam = rk4_step(P, tab, T0, beta, lam0, lam, h);
+    return lam;
+}
+
+// O5: lambda after integrating over tau.  The single-step result is always computed (straight-line code); a cell
+// whose temperature bound reaches Tsafe (n_sub may exceed 1) redoes the integration behind a warp-uniform branch.
 __device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0,
                                                 double tau, double Tsafe)
 {
-    const double Tub = fma(beta, lam0, T0);
-    int nsub = 1;
-    double h = tau;
-    if (Tub >= Tsafe) { nsub = nsub_exact(P, Tub, tau); h = tau / (double)nsub; }
-    const double nTa = P.Ta, mC = -P.Cpre;
-    double lam = lam0;
-    for (int s = 0; s < nsub; ++s) {
-        double l, T, k1, k2, k3, k4;
-        l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = is_pos(T) ? k1 : 0.0;
-        l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = is_pos(T) ? k2 : 0.0;
-        l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = is_pos(T) ? k3 : 0.0;
-        l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = is_pos(T) ? k4 : 0.0;
-        lam = fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
+    double lam = rk4_step(P, tab, T0, beta, lam0, lam0, tau);
+    const bool hot = fma(beta, lam0, T0) >= Tsafe;
+    if (__any_sync(__activemask(), hot)) {
+        const double l2 = rk4_substepped(P, tab, T0, beta, lam0, tau);
+        lam = hot ? l2 : lam;
     }
     return dmin_(nonneg(lam), lam0);
 }
@@ -189,8 +205,12 @@ __device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double
     const double SR = dmax_(L.un + L.c, R.un + R.c);
     const double mL = L.rho * (SL - L.un), mR = R.rho * (SR - R.un);
     const double Sstar = (R.p - L.p + fma(L.un, mL, -R.un * mR)) * q_rcp(mL - mR);
-    const bool useL = (SL >= 0.0) || ((SR > 0.0) && (Sstar >= 0.0));
-    const bool star = (SL < 0.0) && (SR > 0.0);
+    // sign tests on the high words (integer pipe).  They differ from the floating-point comparisons only for -0.0 and
+    // subnormals: SL = -0.0 enters the star branch with SKs = -0.0, where F* = F_L exactly; S* = -0.0 takes the right
+    // star state, whose flux equals the left one at S* = 0 (F*_L - F*_R = S* (U*_L - U*_R)); a subnormal SR counts as 0.
+    const bool sl_neg = hi_word(SL) < 0, sr_pos = hi_word(SR) > 0;
+    const bool useL = !sl_neg || (sr_pos && hi_word(Sstar) >= 0);
+    const bool star = sl_neg && sr_pos;
     const double r1 = useL ? L.r1 : R.r1, r2 = useL ? L.r2 : R.r2, un = useL ? L.un : R.un, ut = useL ? L.ut : R.ut;
     const double p = useL ? L.p : R.p, z1 = useL ? L.z1 : R.z1, lam = useL ? L.lam : R.lam;
     const double rho = useL ? L.rho : R.rho, rhoE = useL ? L.rhoE : R.rhoE, SK = useL ? SL : SR;
