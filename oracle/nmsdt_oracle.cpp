@@ -755,3 +755,81 @@ extern "C" int orc_read_field(orc_t* s, int id, double* out)
         }
     return 0;
 }
+
+/* ============================ post-processing ================ */
+
+extern "C" int orc_profiles(orc_t* s, double p_front, double* pbar, double* rhobar, double* ubar, double* xs_out)
+{   /* Eq. 9-11, Appendix C front position; R23, R25 */
+    if (!s || !s->inited) return -3;
+    const int nx = s->g.nx, ny = s->g.ny;
+    int front = -1;
+    for (int i = 0; i < nx; ++i) {
+        double sp = 0.0, sr = 0.0, sm = 0.0;
+        for (int j = 0; j < ny; ++j) {
+            size_t id = s->idx(i, j);
+            double q[7], W[7], c, T2;
+            for (int f = 0; f < 7; ++f) q[f] = s->q[f][id];
+            orc_cons_to_prim(&s->e, q, W, &c, &T2);
+            sp += W[4];
+            sr += q[0] + q[1];
+            sm += q[2];
+        }
+        const double pb = sp / (double)ny;
+        if (pbar) pbar[i] = pb;
+        if (rhobar) rhobar[i] = sr / (double)ny;
+        if (ubar) ubar[i] = sm / sr;
+        if (pb >= p_front) front = i;
+    }
+    if (xs_out) *xs_out = s->g.dx * (double)(front + 1);
+    return 0;
+}
+
+extern "C" int orc_qdot_pdf(orc_t* s, double n_lo, double dn, int nbins, double* mass, long long* count)
+{   /* Eq. 14-16; R24 */
+    if (!s || !s->inited || nbins < 1 || !(dn > 0.0)) return -3;
+    const int nx = s->g.nx, ny = s->g.ny;
+    const double dA = s->g.dx * s->g.dy;
+    for (int b = 0; b < nbins; ++b) { if (mass) mass[b] = 0.0; if (count) count[b] = 0; }
+    if (!s->k.reactive) return 0;
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            size_t id = s->idx(i, j);
+            double q[7], W[7], c, T2;
+            for (int f = 0; f < 7; ++f) q[f] = s->q[f][id];
+            orc_cons_to_prim(&s->e, q, W, &c, &T2);
+            if (!(T2 > 0.0)) continue;
+            const double qdot = q[6] * s->k.Cpre * std::exp(-s->k.Ta / T2) * s->k.Q;     /* Eq. 14, W/m^3 */
+            if (!(qdot > 0.0)) continue;
+            const double n = std::log10(qdot / 1e9);                                     /* Eq. 15, GW/m^3 */
+            const double fb = std::floor((n - n_lo) / dn);
+            if (fb < 0.0 || fb >= (double)nbins) continue;
+            const int b = (int)fb;
+            if (mass) mass[b] += q[1] * dA;
+            if (count) count[b] += 1;
+        }
+    return 0;
+}
+
+static double interp_linear(const double* t, const double* x, int n, double tq, bool* ok)
+{
+    if (!(tq >= t[0]) || !(tq <= t[n - 1])) { *ok = false; return 0.0; }
+    int k = 0;
+    while (k < n - 2 && t[k + 1] < tq) ++k;                 /* t[k] <= tq <= t[k+1] */
+    const double w = (tq - t[k]) / (t[k + 1] - t[k]);
+    return x[k] + w * (x[k + 1] - x[k]);
+}
+
+extern "C" int orc_shock_kinematics(const double* t, const double* xs, int n, double dtau, double* us, double* as)
+{   /* Eq. C1-C2; R26 */
+    if (!t || !xs || n < 2 || !(dtau > 0.0)) return -1;
+    const double nan = std::nan("");
+    for (int k = 0; k < n; ++k) {
+        bool ok = true;
+        const double xp = interp_linear(t, xs, n, t[k] + 0.5 * dtau, &ok), xm = interp_linear(t, xs, n, t[k] - 0.5 * dtau, &ok);
+        if (us) us[k] = ok ? (xp - xm) / dtau : nan;
+        ok = true;
+        const double xpp = interp_linear(t, xs, n, t[k] + dtau, &ok), xmm = interp_linear(t, xs, n, t[k] - dtau, &ok);
+        if (as) as[k] = ok ? (xpp - 2.0 * xs[k] + xmm) / (dtau * dtau) : nan;
+    }
+    return 0;
+}

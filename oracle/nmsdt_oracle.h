@@ -86,6 +86,21 @@ int  orc_read_field(orc_t*, int field_id, double* out);
 int  orc_get_cavities(orc_t*, orc_cavity_t* out, int cap, int* n);
 long long orc_fallback_count(orc_t*);              /* number of first-order fallbacks so far */
 
+/* ---- post-processing of the paper's figures (readings R23-R26 of DESIGN.md) --------------
+ * orc_profiles: Eq. 9-11 by the midpoint rule on the uniform grid, plain sequential sums over j:
+ *   pbar_i = (1/ny) sum_j p_ij,  rhobar_i = (1/ny) sum_j rho_ij,  ubar_i = sum_j (rho u)_ij / sum_j rho_ij,
+ *   and the leading-shock position of Appendix C: x_s = dx * (1 + max{i : pbar_i >= p_front}), 0 if none
+ *   (the paper's p_front is 1.01 p0).  Any output pointer may be NULL.
+ * orc_qdot_pdf: Eq. 14-16: qdot = q6 C exp(-Ta/T2) Q [W/m^3] (0 when inert or T2 <= 0),
+ *   n = log10(qdot / 1e9), bin b = floor((n - n_lo)/dn) counted iff 0 <= b < nbins; mass[b] += q1 dx dy (the mass of NM
+ *   in the cell), count[b] += 1.  Eq. 16's f = mass / (M2tot0 dn) is left to the caller.
+ * orc_shock_kinematics: Eq. C1-C2 on samples (t_k, xs_k) with x_s(t) interpolated linearly between
+ *   samples: us_k = [x_s(t_k + dtau/2) - x_s(t_k - dtau/2)]/dtau, as_k = [x_s(t_k + dtau) - 2 x_s(t_k) + x_s(t_k - dtau)]/dtau^2
+ *   (C1 substituted into C2); NaN where the window leaves [t_0, t_{n-1}]. */
+int  orc_profiles(orc_t*, double p_front, double* pbar, double* rhobar, double* ubar, double* xs_out);
+int  orc_qdot_pdf(orc_t*, double n_lo, double dn, int nbins, double* mass, long long* count);
+int  orc_shock_kinematics(const double* t, const double* xs, int n, double dtau, double* us, double* as);
+
 /* ---- pieces of the step, exposed so that tests can pin them one by one ----------- */
 int  orc_halo(orc_t*, int dir);                    /* fill ghosts for a sweep in dir (0 = x, 1 = y) */
 int  orc_sweep(orc_t*, int dir, double dt);        /* halo + one directional MUSCL-Hancock/HLLC sweep */

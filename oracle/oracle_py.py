@@ -90,6 +90,9 @@ def lib():
             ("orc_step_dt", C.c_int, [C.c_void_p, C.c_int, C.c_double]),
             ("orc_diagnostics", C.c_int, [C.c_void_p, C.POINTER(Diag)]),
             ("orc_read_field", C.c_int, [C.c_void_p, C.c_int, dp]),
+            ("orc_profiles", C.c_int, [C.c_void_p, C.c_double, dp, dp, dp, dp]),
+            ("orc_qdot_pdf", C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_int, dp, C.POINTER(C.c_longlong)]),
+            ("orc_shock_kinematics", C.c_int, [dp, dp, C.c_int, C.c_double, dp, dp]),
             ("orc_get_cavities", C.c_int, [C.c_void_p, C.POINTER(Cavity), C.c_int, C.POINTER(C.c_int)]),
             ("orc_fallback_count", C.c_longlong, [C.c_void_p]),
             ("orc_halo", C.c_int, [C.c_void_p, C.c_int]),
@@ -207,6 +210,21 @@ class Oracle:
         self._chk(self.L.orc_read_field(self.h, int(fid), _dp(out)), "orc_read_field")
         return out
 
+    def profiles(self, p_front):
+        """Eq. 9-11 and the Appendix C front position: (pbar[nx], rhobar[nx], ubar[nx], x_s)"""
+        pb, rb, ub = (np.empty(self.nx, dtype=np.float64) for _ in range(3))
+        xs = C.c_double()
+        self._chk(self.L.orc_profiles(self.h, float(p_front), _dp(pb), _dp(rb), _dp(ub), C.byref(xs)), "orc_profiles")
+        return pb, rb, ub, xs.value
+
+    def qdot_pdf(self, n_lo=2.0, dn=0.02, nbins=400):
+        """Eq. 14-16: (mass[nbins], count[nbins])"""
+        m = np.empty(nbins, dtype=np.float64)
+        c = np.empty(nbins, dtype=np.int64)
+        self._chk(self.L.orc_qdot_pdf(self.h, float(n_lo), float(dn), int(nbins), _dp(m),
+                                      c.ctypes.data_as(C.POINTER(C.c_longlong))), "orc_qdot_pdf")
+        return m, c
+
     def state(self):
         return [self.read_field(k) for k in range(7)]
 
@@ -268,3 +286,14 @@ def gen_cavities(seed, phi, dmin, dmax, min_gap, x_lo, x_hi, ny, periodic_y, cap
     if n < 0:
         raise RuntimeError("orc_gen_cavities failed")
     return np.array([[arr[i].x, arr[i].y, arr[i].r] for i in range(n)], dtype=np.float64).reshape(-1, 3)
+
+
+def shock_kinematics(t, xs, dtau):
+    """Eq. C1-C2: (u_s[n], a_s[n]), NaN where the window leaves the sampled interval"""
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    xs = np.ascontiguousarray(xs, dtype=np.float64)
+    us, a = np.empty_like(t), np.empty_like(t)
+    rc = lib().orc_shock_kinematics(_dp(t), _dp(xs), int(t.size), float(dtau), _dp(us), _dp(a))
+    if rc != 0:
+        raise RuntimeError("orc_shock_kinematics failed: %d" % rc)
+    return us, a
