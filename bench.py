@@ -30,15 +30,15 @@ from paper_1905_05727_b200 import inputs  # noqa: E402
 METRIC = "fp64 cell-updates/s per 2D step"
 UNIT = "cell-updates/s"
 # algorithmic FP64 work of one cell in one fused directional sweep, from ncu's counters of the
-# C5 launches (profiles/r01b_fused_c5.md) divided by the 33/32 ramp-up redundancy of a segment.
+# C5 launches (profiles/r01c_fused_c5.md) divided by the 33/32 ramp-up redundancy of a segment.
 #   FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot):
-FP64_INSTR_PER_CELL = {"lead": 455.0, "trail": 546.0}       # pass 1 = S + sweep; pass 2 = sweep + S + wavespeed
-#   flops with dadd = dmul = 1, dfma = 2 (56 % of the FP64 instructions are DFMA):
-FLOP_PER_CELL = {"lead": 648.0, "trail": 776.0}
+FP64_INSTR_PER_CELL = {"lead": 407.0, "trail": 489.0}       # pass 1 = S + sweep; pass 2 = sweep + S + wavespeed
+#   flops with dadd = dmul = 1, dfma = 2 (52 % of the FP64 instructions are DFMA):
+FLOP_PER_CELL = {"lead": 602.0, "trail": 718.0}
 FP64_LANES_PER_SM, N_SM = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per cell per launch from the ncu --set full capture of C5 (mean of the
-# lead and trail launches; profiles/r01b_fused_c5.md): 113.6 B (x), 113.6 B (y) against 112 B algorithmic
-TRAFFIC_BYTES_PER_CELL = {"sweep_x": 113.8, "sweep_y": 113.6}
+# lead and trail launches; profiles/r01c_fused_c5.md): 112.9 B (x), 112.9 B (y) against 112 B algorithmic
+TRAFFIC_BYTES_PER_CELL = {"sweep_x": 112.9, "sweep_y": 112.9}
 
 
 def peaks():
@@ -228,6 +228,19 @@ def main():
             "hbm_peak_gbs": pk.get("hbm_gbs", 6650.0),
             "kernel_ms_per_step": {k: v[0] / K for k, v in kt.items()}}
 
+    # ---- post-processing calls (not part of a step): one state read each, HBM bound ----------------
+    post = {}
+    for name, fn, planes in (("profiles", lambda: sim.profiles(1.01 * cfg["init"]["p0"]), 6), ("qdot_pdf", lambda: sim.qdot_pdf(), 7),
+                             ("diagnostics", lambda: sim.diagnostics(), 7)):
+        fn()
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(3):
+            t0 = time.perf_counter()
+            fn()                                   # [sync] calls: kernels + a few KB back to the host
+            best = min(best, time.perf_counter() - t0)
+        post[name] = {"ms": best * 1e3, "hbm_gbs_algorithmic": planes * 8 * cells / best / 1e9}
+
     # ---- end to end through the C ABI with host buffers -------------------------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -271,6 +284,7 @@ def main():
                    "variant": args.variant, "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "burned_mass": d["burned_mass"]},
+        "post": post,
     }
     print(json.dumps(out))
     if world > 1:

@@ -132,6 +132,24 @@ int sim_read_field(sim_t*, int field_id, double* host_out);
 /* Cavity list used by the last sim_init (generator parity). Writes min(n, cap) entries. [sync] */
 int sim_get_cavities(sim_t*, sim_cavity_t* host_out, int cap, int* n);
 
+/* ---- post-processing of the state (the paper's analysis figures; R23-R26).  Not part of sim_step. ----
+ * sim_profiles: y-averaged profiles Eq. 9-11 by the midpoint rule over the ny rows,
+ *     pbar_i = (1/ny) sum_j p_ij,  rhobar_i = (1/ny) sum_j rho_ij,  ubar_i = sum_j (rho u)_ij / sum_j rho_ij,
+ *   into HOST arrays of nx doubles (any of them may be NULL), and the leading-shock position of Appendix C,
+ *     *xs_out = dx * (1 + max{i : pbar_i >= p_front})  [m], 0 if no column reaches p_front (the paper uses 1.01 p0).
+ * sim_qdot_pdf: mass-weighted histogram of the volumetric energy-release rate, Eq. 14-16:
+ *     qdot = q6 C exp(-Ta/T2) Q [W/m^3];  n = log10(qdot / 1e9);  b = floor((n - n_lo)/dn), counted iff 0 <= b < nbins;
+ *     host_mass[b] += q1 dx dy  (mass of NM in the cell per unit depth),  host_count[b] += 1.
+ *   Eq. 16's f = host_mass / (M2tot0 dn) is one division by the caller.  The paper's window is n_lo = 2, dn = 0.02,
+ *   nbins = 400.  1 <= nbins <= 1024; either HOST output may be NULL.  An inert run returns zeros.
+ * sim_shock_kinematics: Eq. C1-C2 on n HOST samples (host_t increasing, host_xs) with x_s(t) interpolated
+ *   linearly: us_k = [x_s(t_k + dtau/2) - x_s(t_k - dtau/2)]/dtau, as_k = [x_s(t_k + dtau) - 2 x_s(t_k) + x_s(t_k - dtau)]/dtau^2,
+ *   NaN where the window leaves [t_0, t_{n-1}].  n >= 2, dtau > 0 (the paper uses 1.5 us).
+ * All three are [sync], deterministic (fixed summation shape) and allocate their scratch inside the library. */
+int sim_profiles(sim_t*, double p_front, double* host_pbar, double* host_rhobar, double* host_ubar, double* xs_out);
+int sim_qdot_pdf(sim_t*, double n_lo, double dn, int nbins, double* host_mass, long long* host_count);
+int sim_shock_kinematics(sim_t*, const double* host_t, const double* host_xs, int n, double dtau, double* host_us, double* host_as);
+
 /* Select kernel variant (SIM_VARIANT_*) and whether sim_step replays CUDA graphs (default on). */
 int sim_set_variant(sim_t*, int variant, int use_graph);
 /* Number of kernel launches enqueued by this handle so far (bench.py's gpu_launches). */

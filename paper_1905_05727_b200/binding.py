@@ -22,7 +22,8 @@ FIELD = {"q0": 0, "q1": 1, "q2": 2, "q3": 3, "q4": 4, "q5": 5, "q6": 6, "p": 16,
 SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error", "sim_init", "sim_init_fields",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
            "sim_read_field", "sim_get_cavities", "sim_set_variant", "sim_launch_count", "sim_device_layout",
-           "sim_probe_fp64", "sim_probe_math", "sim_profile", "sim_kernel_time"]
+           "sim_probe_fp64", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
+           "sim_shock_kinematics"]
 KERNEL_KINDS = {"sweep_x": 0, "sweep_y": 1, "source": 2, "cfl": 3, "halo": 4}
 
 
@@ -101,6 +102,9 @@ def load_library():
         "sim_device_layout": (C.c_int, [vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(C.c_int),
                                         C.POINTER(C.c_int), C.POINTER(C.c_int)]),
         "sim_probe_fp64": (C.c_int, [vp, dp, dp]),
+        "sim_profiles": (C.c_int, [vp, C.c_double, dp, dp, dp, dp]),
+        "sim_qdot_pdf": (C.c_int, [vp, C.c_double, C.c_double, C.c_int, dp, C.POINTER(C.c_longlong)]),
+        "sim_shock_kinematics": (C.c_int, [vp, dp, dp, C.c_int, C.c_double, dp, dp]),
         "sim_probe_math": (C.c_int, [vp, C.c_int, dp, C.c_int, C.c_double, C.c_double, dp, dp]),
         "sim_profile": (C.c_int, [vp, C.c_int]),
         "sim_kernel_time": (C.c_int, [vp, C.c_int, dp, C.POINTER(C.c_longlong)]),
@@ -243,6 +247,33 @@ class Sim:
         g, ms = C.c_double(), C.c_double()
         self._chk(self.L.sim_probe_fp64(self.h, C.byref(g), C.byref(ms)), "sim_probe_fp64")
         return g.value, ms.value
+
+    def profiles(self, p_front):
+        """Eq. 9-11 and the Appendix C front position: (pbar[nx], rhobar[nx], ubar[nx], x_s)"""
+        dp = C.POINTER(C.c_double)
+        pb, rb, ub = (np.empty(self.nx, dtype=np.float64) for _ in range(3))
+        xs = C.c_double()
+        self._chk(self.L.sim_profiles(self.h, float(p_front), pb.ctypes.data_as(dp), rb.ctypes.data_as(dp),
+                                      ub.ctypes.data_as(dp), C.byref(xs)), "sim_profiles")
+        return pb, rb, ub, xs.value
+
+    def qdot_pdf(self, n_lo=2.0, dn=0.02, nbins=400):
+        """Eq. 14-16: (mass[nbins], count[nbins])"""
+        m = np.empty(nbins, dtype=np.float64)
+        c = np.empty(nbins, dtype=np.int64)
+        self._chk(self.L.sim_qdot_pdf(self.h, float(n_lo), float(dn), int(nbins), m.ctypes.data_as(C.POINTER(C.c_double)),
+                                      c.ctypes.data_as(C.POINTER(C.c_longlong))), "sim_qdot_pdf")
+        return m, c
+
+    def shock_kinematics(self, t, xs, dtau):
+        """Eq. C1-C2: (u_s[n], a_s[n])"""
+        dp = C.POINTER(C.c_double)
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        xs = np.ascontiguousarray(xs, dtype=np.float64)
+        us, a = np.empty_like(t), np.empty_like(t)
+        self._chk(self.L.sim_shock_kinematics(self.h, t.ctypes.data_as(dp), xs.ctypes.data_as(dp), int(t.size), float(dtau),
+                                              us.ctypes.data_as(dp), a.ctypes.data_as(dp)), "sim_shock_kinematics")
+        return us, a
 
     def probe_math(self, fn, x, a=0.0, b=0.0):
         """device evaluation of the fused path's elementary functions (include/nmsdt.h: sim_probe_math)"""

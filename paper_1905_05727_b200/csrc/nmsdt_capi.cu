@@ -59,6 +59,8 @@ struct sim {
     Ctl* ctl = nullptr;
     Cav* d_cav = nullptr;
     int ncav = 0;
+    double* post = nullptr;         // scratch of the post-processing calls (library-owned, grown on demand)
+    size_t post_bytes = 0;
     bool inited = false;
     long long host_step = 0;        // mirrors ctl->step (step parity decides the sweep order)
     double M2tot0 = 0.0;
@@ -318,6 +320,7 @@ void sim_destroy(sim_t* s)
     if (!s) return;
     cudaStreamSynchronize(s->stream);
     if (s->d_cav) cudaFree(s->d_cav);
+    if (s->post) cudaFree(s->post);
     if (s->gexec) cudaGraphExecDestroy(s->gexec);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     for (auto& p : s->ev) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
@@ -574,6 +577,69 @@ int sim_probe_fp64(sim_t* s, double* gflops_out, double* ms_out)
     int rc = launch_probe_fp64(s->stream, gflops_out, ms_out);
     if (rc) return fail(s, SIM_ERR_CUDA, "sim_probe_fp64 failed");
     return SIM_OK;
+}
+
+namespace {
+// library-owned scratch for the post-processing calls
+double* post_scratch(sim* s, size_t bytes)
+{
+    if (bytes > s->post_bytes) {
+        if (s->post) { cudaStreamSynchronize(s->stream); cudaFree(s->post); s->post = nullptr; s->post_bytes = 0; }
+        if (cudaMalloc(&s->post, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        s->post_bytes = bytes;
+    }
+    return s->post;
+}
+} // namespace
+
+int sim_profiles(sim_t* s, double p_front, double* host_pbar, double* host_rhobar, double* host_ubar, double* xs_out)
+{
+    if (!s) return fail(s, SIM_ERR_ARG, "sim_profiles: NULL handle");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_profiles: not initialised");
+    double* buf = post_scratch(s, post_profiles_bytes(s->g.nx, s->g.ny));
+    if (!buf) return fail(s, SIM_ERR_CUDA, "sim_profiles: cannot allocate scratch");
+    double *d_out = nullptr, *d_xs = nullptr;
+    s->launches += launch_profiles(s->P, s->A, p_front, buf, &d_out, &d_xs, s->stream);
+    const size_t nb = (size_t)s->g.nx * sizeof(double);
+    if (host_pbar) cudaMemcpyAsync(host_pbar, d_out, nb, cudaMemcpyDeviceToHost, s->stream);
+    if (host_rhobar) cudaMemcpyAsync(host_rhobar, d_out + s->g.nx, nb, cudaMemcpyDeviceToHost, s->stream);
+    if (host_ubar) cudaMemcpyAsync(host_ubar, d_out + 2 * (size_t)s->g.nx, nb, cudaMemcpyDeviceToHost, s->stream);
+    if (xs_out) cudaMemcpyAsync(xs_out, d_xs, sizeof(double), cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_profiles");
+    return check_cuda(s, "sim_profiles");
+}
+
+int sim_qdot_pdf(sim_t* s, double n_lo, double dn, int nbins, double* host_mass, long long* host_count)
+{
+    if (!s || !(dn > 0.0) || nbins < 1 || nbins > POST_MAX_BINS) return fail(s, SIM_ERR_ARG, "sim_qdot_pdf: bad argument (1 <= nbins <= 1024, dn > 0)");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_qdot_pdf: not initialised");
+    if (!s->P.reactive) {                       // inert run: no energy release, empty statistics
+        for (int b = 0; b < nbins; ++b) { if (host_mass) host_mass[b] = 0.0; if (host_count) host_count[b] = 0; }
+        return SIM_OK;
+    }
+    double* buf = post_scratch(s, post_hist_bytes(nbins));
+    if (!buf) return fail(s, SIM_ERR_CUDA, "sim_qdot_pdf: cannot allocate scratch");
+    double* d_mass = nullptr; unsigned long long* d_count = nullptr;
+    s->launches += launch_qdot_hist(s->P, s->A, n_lo, dn, nbins, buf, &d_mass, &d_count, s->stream);
+    if (host_mass) cudaMemcpyAsync(host_mass, d_mass, sizeof(double) * nbins, cudaMemcpyDeviceToHost, s->stream);
+    if (host_count) cudaMemcpyAsync(host_count, d_count, sizeof(long long) * nbins, cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_qdot_pdf");
+    return check_cuda(s, "sim_qdot_pdf");
+}
+
+int sim_shock_kinematics(sim_t* s, const double* host_t, const double* host_xs, int n, double dtau, double* host_us, double* host_as)
+{
+    if (!s || !host_t || !host_xs || !host_us || !host_as || n < 2 || !(dtau > 0.0)) return fail(s, SIM_ERR_ARG, "sim_shock_kinematics: bad argument");
+    double* buf = post_scratch(s, 4 * (size_t)n * sizeof(double));
+    if (!buf) return fail(s, SIM_ERR_CUDA, "sim_shock_kinematics: cannot allocate scratch");
+    const size_t nb = (size_t)n * sizeof(double);
+    cudaMemcpyAsync(buf, host_t, nb, cudaMemcpyHostToDevice, s->stream);
+    cudaMemcpyAsync(buf + n, host_xs, nb, cudaMemcpyHostToDevice, s->stream);
+    s->launches += launch_kinematics(buf, buf + n, n, dtau, buf + 2 * (size_t)n, buf + 3 * (size_t)n, s->stream);
+    cudaMemcpyAsync(host_us, buf + 2 * (size_t)n, nb, cudaMemcpyDeviceToHost, s->stream);
+    cudaMemcpyAsync(host_as, buf + 3 * (size_t)n, nb, cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_shock_kinematics");
+    return check_cuda(s, "sim_shock_kinematics");
 }
 
 int sim_probe_math(sim_t* s, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1)

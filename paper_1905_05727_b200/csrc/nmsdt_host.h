@@ -39,6 +39,17 @@ double host_tsafe(double tau, double Cpre, double Ta, double theta0);
 int  launch_probe_math(const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
                        cudaStream_t s);
 
+// post-processing (nmsdt_post.cu): Eq. 9-11 profiles + front position, Eq. 14-16 histogram, Eq. C1-C2 kinematics.
+// Each launcher returns the number of kernels it enqueued.
+constexpr int POST_HIST_BLOCKS = 592;      // 4 x 148
+constexpr int POST_MAX_BINS = 1024;
+size_t post_profiles_bytes(int nx, int ny);
+size_t post_hist_bytes(int nbins);
+int launch_profiles(const Params& P, const double* q, double p_front, double* buf, double** d_out, double** d_xs, cudaStream_t s);
+int launch_qdot_hist(const Params& P, const double* q, double n_lo, double dn, int nbins, double* buf, double** d_mass,
+                     unsigned long long** d_count, cudaStream_t s);
+int launch_kinematics(const double* d_t, const double* d_xs, int n, double dtau, double* d_us, double* d_as, cudaStream_t s);
+
 // init / output kernels (nmsdt_init.cu)
 void launch_zero_plane(const Params& P, double* plane, cudaStream_t s);
 void launch_paint(const Params& P, double* prof_plane, const Cav* cav, int ncav, double h, cudaStream_t s);
