@@ -103,6 +103,22 @@ def oracle_rate(cfg_name, budget_s=12.0, crop=(2048, 512)):
         cfg_name, crop[0], crop[1], n, el, cores), el / n
 
 
+def max_over_ranks(x, world, device):
+    """the slowest rank's time (the bench contract times the job as the max over ranks); nccl on GPU, gloo on CPU"""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(cells, steps, world, seconds_max):
+    """whole-job throughput of `world` independent replicas (replicas only): units all ranks processed / max time"""
+    return cells * steps * world / seconds_max
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -190,11 +206,8 @@ def main():
     sampler.join(timeout=2)
     kt = sim.kernel_times()
     d = sim.diagnostics()
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = cells * K * world / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, "cuda")
+    value = aggregate_value(cells, K, world, ms * 1e-3)
 
     # ---- roofline of the dominant kernel --------------------------------------------------------------------
     # The sweeps are bound by the FP64 pipe: one warp instruction per 2 clocks per SMSP whatever the
@@ -260,12 +273,9 @@ def main():
             sim.read_field_into(k, views[k])       # D2H of the result fields
         barrier()
         el = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([el], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
+        el = max_over_ranks(el, world, "cuda")
         nbytes = 7 * cells * 8
-        e2e = {"value": cells * K * world / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
+        e2e = {"value": aggregate_value(cells, K, world, el), "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
                "job": "sim_init_fields(host) + sim_step(%d) + sim_diagnostics + 7 x sim_read_field(host)" % K, "seconds": el,
                "M2r": de["M2r"]}
 

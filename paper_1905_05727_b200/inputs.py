@@ -80,3 +80,33 @@ def config(name, p_shock=None, reactive=None, nx=None, ny=None, seed=None):
     if seed is not None:
         init["seed"] = int(seed)
     return dict(name=name, grid=grid, eos=eos, kin=kin, init=init, steps=steps)
+
+
+def paper_case(case, dx_um=1.0, p_shock=7.81e9, phi=None, seed=2019, length_mm=24.0):
+    """The paper's own scenarios (Sect. IV, Appendix A) at grid spacing dx_um (paper: 1 um; Tables IV-V also
+    give 4 and 2 um): 'neat' (W arbitrary: 32 cells), 'regular' (one row of d_c = 100 um cavities, W = delta_c of Eq. 7,
+    phi = 8 %), 'random' (W = 2 mm, centre spacing >= 2.5 d_c, phi = 5 % as in Table V or 8 % as in Sect. IV).
+    Domain length 24 mm, shocked slab L_s = 0.5 mm, input shock 7.81 GPa, periodic top / bottom."""
+    import math
+    eos, kin, init = copy.deepcopy(EOS), copy.deepcopy(KIN), copy.deepcopy(_INIT0)
+    dx = dx_um * 1e-6
+    nx = int(round(length_mm * 1e-3 / dx))
+    ls = int(round(0.5e-3 / dx))
+    dc = 100e-6 / dx                                   # cavity diameter in cells
+    init.update(p_shock=float(p_shock), shock_cells=ls)
+    if case == "neat":
+        ny = 32
+    elif case == "regular":
+        phi = 0.08 if phi is None else phi
+        delta = math.sqrt(math.pi * dc * dc / (4.0 * phi))            # Eq. 7, in cells
+        ny = int(round(delta))
+        # one row of cavities on the axis of a strip of width ny ~ delta (periodic images at distance ny), spacing delta in x
+        ncol = int((nx - ls) / delta)
+        init.update(cavities=[(ls + 0.5 * delta + delta * i, 0.5 * ny, 0.5 * dc) for i in range(ncol)])
+    elif case == "random":
+        phi = 0.05 if phi is None else phi
+        ny = int(round(2.0e-3 / dx))
+        init.update(seed=int(seed), phi=float(phi), dmin=dc, dmax=dc, min_gap=1.5 * dc, x_lo=ls, x_hi=nx)
+    else:
+        raise ValueError("unknown paper case %r" % (case,))
+    return dict(name="paper-%s-dx%g" % (case, dx_um), grid=_grid(nx, ny, dx), eos=eos, kin=kin, init=init, steps=0)
