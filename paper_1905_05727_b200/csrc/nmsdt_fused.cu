@@ -75,7 +75,11 @@ __device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* _
 {
     double lam = rk4_step(P, tab, T0, beta, lam0, lam0, tau);
     const bool hot = fma(beta, lam0, T0) >= Tsafe;
+#if NMSDT_EXP_NOBRANCH
+    if (false) {
+#else
     if (__any_sync(__activemask(), hot)) {
+#endif
         const double l2 = rk4_substepped(P, tab, T0, beta, lam0, tau);
         lam = hot ? l2 : lam;
     }
@@ -184,7 +188,11 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
     // R17 first-order fallback.  It practically never fires, so it sits behind a warp-uniform branch instead of 14
     // unconditional selects.
     const bool ok = min(min(hi_word(WL[0]), hi_word(WL[1])), min(hi_word(WR[0]), hi_word(WR[1]))) > 0;   // all four > 0
+#if NMSDT_EXP_NOBRANCH
+    if (false) {
+#else
     if (__any_sync(__activemask(), !ok)) {
+#endif
 #pragma unroll
         for (int k = 0; k < 7; ++k) { WL[k] = ok ? WL[k] : w0[k]; WR[k] = ok ? WR[k] : w0[k]; }
     }
@@ -277,6 +285,9 @@ __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double la
     }
 }
 
+#ifndef NMSDT_EXP_NOBRANCH
+#define NMSDT_EXP_NOBRANCH 0
+#endif
 #ifndef NMSDT_Y_MINBLOCKS
 #define NMSDT_Y_MINBLOCKS 4
 #endif
