@@ -22,7 +22,9 @@ namespace nmsdt {
 
 namespace {
 
-enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2 };
+// pass kinds: PLAIN = sweep only; LEAD = S(dt/2) on load + sweep; TRAIL = sweep + S(dt/2) + wavespeed of the new state;
+// TRAIL_INERT = sweep + wavespeed (inert runs: pass 1 is PLAIN, pass 2 is TRAIL_INERT)
+enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2, MODE_TRAIL_INERT = 3 };
 
 struct FCell {            // W = (rho1, rho2, un, ut, p, z1, lambda) + what the Hancock predictor needs
     double r1, r2, un, ut, p, z1, lam;
@@ -68,29 +70,37 @@ __device__ __noinline__ double rk4_substepped(const Params& P, const double* __r
     return lam;
 }
 
-// O5: lambda after integrating over tau.  The single-step result is always computed (straight-line code); a cell
-// whose temperature bound reaches Tsafe (n_sub may exceed 1) redoes the integration behind a warp-uniform branch.
+// O5: lambda after integrating over tau.
+// SRC_FAST: one RK4 step, straight-line code; `hot` is raised when the temperature bound reaches Tsafe, i.e. when the
+// R13 rule could ask for more than one sub-step: the caller then redoes its whole segment with SRC_EXACT.  Keeping
+// this decision out of the marching loop keeps the loop body one basic block (the serial RK4 chain overlaps with
+// the EOS evaluations of the faces).
+// SRC_EXACT: the R13 rule, sub-stepped integration behind a warp-uniform branch.
+enum { SRC_NONE = 0, SRC_FAST = 1, SRC_EXACT = 2 };
+template <int SRC>
 __device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0,
-                                                double tau, double Tsafe)
+                                                double tau, double Tsafe, bool& hot)
 {
     double lam = rk4_step(P, tab, T0, beta, lam0, lam0, tau);
-    const bool hot = fma(beta, lam0, T0) >= Tsafe;
-#if NMSDT_EXP_NOBRANCH
-    if (false) {
-#else
-    if (__any_sync(__activemask(), hot)) {
-#endif
-        const double l2 = rk4_substepped(P, tab, T0, beta, lam0, tau);
-        lam = hot ? l2 : lam;
+    const bool h = fma(beta, lam0, T0) >= Tsafe;
+    if (SRC == SRC_FAST) {
+        hot |= h;
+    } else {
+        if (__any_sync(__activemask(), h)) {
+            const double l2 = rk4_substepped(P, tab, T0, beta, lam0, tau);
+            lam = h ? l2 : lam;
+        }
     }
     return dmin_(nonneg(lam), lam0);
 }
 
 // O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.
 // SRC: the Arrhenius step over tau is applied to the cell; dE = energy moved into rho E, q6n = new z2 rho2 lambda.
-template <bool SRC>
+// The kernels that apply the source are only launched for reactive runs (launch_sweep_fused), so there is no
+// P.reactive test here.
+template <int SRC>
 __device__ __forceinline__ void prim_cell(const Params& P, const double* __restrict__ tab, const double q[7], double tau, double Tsafe,
-                                          FCell& W, double& dE, double& q6n)
+                                          FCell& W, double& dE, double& q6n, bool& hot)
 {
     const double rho = q[0] + q[1];
     const double irho = q_rcp(rho);
@@ -114,16 +124,14 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     double p = (rhoe - z2 * fma(-pr, P.iG2, rer)) * ixi;
     double lam = clamp01(q[6] * iq1);
     dE = 0.0; q6n = q[6];
-    if (SRC) {
-        if (P.reactive) {
-            const double T0 = P.Tref2 + (p - pr) * (z2 * iq1) * P.iG2cv2;        // Eq. 5 (1/rho2 = z2/q1)
-            const double beta = z2 * P.Q * ixi * P.iG2cv2;
-            const double lam1 = arrhenius_rk4(P, tab, T0, beta, lam, tau, Tsafe);
-            dE = q[1] * P.Q * (lam - lam1);
-            q6n = q[1] * lam1;
-            p = fma(dE, ixi, p);                                                 // p is linear in rho e at frozen rho_k, z_k
-            lam = lam1;
-        }
+    if (SRC != SRC_NONE) {
+        const double T0 = P.Tref2 + (p - pr) * (z2 * iq1) * P.iG2cv2;            // Eq. 5 (1/rho2 = z2/q1)
+        const double beta = z2 * P.Q * ixi * P.iG2cv2;
+        const double lam1 = arrhenius_rk4<SRC>(P, tab, T0, beta, lam, tau, Tsafe, hot);
+        dE = q[1] * P.Q * (lam - lam1);
+        q6n = q[1] * lam1;
+        p = fma(dE, ixi, p);                                                     // p is linear in rho e at frozen rho_k, z_k
+        lam = lam1;
     }
     W.p = p; W.lam = lam;
     const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
@@ -162,7 +170,10 @@ __device__ __forceinline__ double limited_f(int kind, double a, double b)
     return a * b > 0.0 ? m : 0.0;
 }
 
-// O4.1-2 for the centre cell W0, given the one-sided differences a = W0 - W(-1), b = W(+1) - W0
+// O4.1-2 for the centre cell W0, given the one-sided differences a = W0 - W(-1), b = W(+1) - W0.
+// R17 first-order fallback (a predicted face density <= 0 -> WL = WR = W0) without a branch: the four densities are
+// predicted first; if one of them is not positive they are replaced by the cell values and the other five slopes are
+// zeroed, which makes their face values equal the cell values exactly (fma(+-0.5, 0, fma(-k, 0, w)) = w).
 __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, const double a[7], const double b[7], double khalf, double WL[7],
                                            double WR[7])
 {
@@ -171,30 +182,29 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
 #pragma unroll
     for (int k = 0; k < 7; ++k) D[k] = limited_f(P.limiter, a[k], b[k]);
     const double u = W0.un;
+    {
+        const double m0 = fma(-khalf, fma(u, D[0], W0.r1 * D[2]), w0[0]);
+        const double m1 = fma(-khalf, fma(u, D[1], W0.r2 * D[2]), w0[1]);
+        WL[0] = fma(-0.5, D[0], m0); WR[0] = fma(0.5, D[0], m0);
+        WL[1] = fma(-0.5, D[1], m1); WR[1] = fma(0.5, D[1], m1);
+    }
+    // all four > 0 (a positive subnormal counts as zero)
+    const bool ok = min(min(hi_word(WL[0]), hi_word(WL[1])), min(hi_word(WR[0]), hi_word(WR[1]))) > 0;
+    WL[0] = ok ? WL[0] : w0[0]; WR[0] = ok ? WR[0] : w0[0];
+    WL[1] = ok ? WL[1] : w0[1]; WR[1] = ok ? WR[1] : w0[1];
+#pragma unroll
+    for (int k = 2; k < 7; ++k) D[k] = ok ? D[k] : 0.0;
     double d[7];
-    d[0] = fma(u, D[0], W0.r1 * D[2]);
-    d[1] = fma(u, D[1], W0.r2 * D[2]);
     d[2] = fma(u, D[2], D[4] * W0.irho);
     d[3] = u * D[3];
     d[4] = fma(u, D[4], W0.rc2 * D[2]);
     d[5] = u * D[5];
     d[6] = u * D[6];
 #pragma unroll
-    for (int k = 0; k < 7; ++k) {
+    for (int k = 2; k < 7; ++k) {
         const double m = fma(-khalf, d[k], w0[k]);
         WL[k] = fma(-0.5, D[k], m);
         WR[k] = fma(0.5, D[k], m);
-    }
-    // R17 first-order fallback.  It practically never fires, so it sits behind a warp-uniform branch instead of 14
-    // unconditional selects.
-    const bool ok = min(min(hi_word(WL[0]), hi_word(WL[1])), min(hi_word(WR[0]), hi_word(WR[1]))) > 0;   // all four > 0
-#if NMSDT_EXP_NOBRANCH
-    if (false) {
-#else
-    if (__any_sync(__activemask(), !ok)) {
-#endif
-#pragma unroll
-        for (int k = 0; k < 7; ++k) { WL[k] = ok ? WL[k] : w0[k]; WR[k] = ok ? WR[k] : w0[k]; }
     }
 }
 
@@ -250,12 +260,13 @@ __device__ __forceinline__ bool all_finite7(const double o[7])
     return m < 0x7ff00000;
 }
 
-// finished cell of the second pass: trailing S(dt/2), wavespeed of the new state, state check (a6, a7, R17)
+// finished cell of the second pass: trailing S(dt/2) (SRC != SRC_NONE), wavespeed of the new state, state check (a6, a7, R17)
+template <int SRC>
 __device__ __forceinline__ void trail_cell(const Params& P, const double* __restrict__ tab, double o[7], double tau, double Tsafe, double& smax,
-                                           int& bad)
+                                           int& bad, bool& hot)
 {
     FCell W; double dE, q6n;
-    prim_cell<true>(P, tab, o, tau, Tsafe, W, dE, q6n);
+    prim_cell<SRC>(P, tab, o, tau, Tsafe, W, dE, q6n, hot);
     o[4] += dE; o[6] = q6n;
     const double a = dmax_(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
     const bool ok = all_finite7(o) && o[0] > 0.0 && o[1] > 0.0 && (__double2hiint(a) & 0x7fffffff) < 0x7ff00000;
@@ -278,16 +289,11 @@ __device__ __forceinline__ void reduce_smax(double smax, int bad, Ctl* ctl)
 // post-source conserved values of a cell whose post-source lambda is known (pass 1 applies S on load, O6)
 __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double lam1)
 {
-    if (P.reactive) {
-        const double q6n = q[1] * lam1;
-        q[4] = fma(P.Q, q[6] - q6n, q[4]);
-        q[6] = q6n;
-    }
+    const double q6n = q[1] * lam1;
+    q[4] = fma(P.Q, q[6] - q6n, q[4]);
+    q[6] = q6n;
 }
 
-#ifndef NMSDT_EXP_NOBRANCH
-#define NMSDT_EXP_NOBRANCH 0
-#endif
 #ifndef NMSDT_Y_MINBLOCKS
 #define NMSDT_Y_MINBLOCKS 4
 #endif
@@ -326,6 +332,111 @@ constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part
 // Per-thread state that lives across rows is kept in thread-private shared-memory slots ([..][YT] layout, conflict
 // free, no barriers): the staged input rows, the primitive window (cells c-2, c-1) and the previous right-face state.
 // Only the half-finished update of cell c-1 stays in registers; this keeps the kernel at 128 registers (16 warps/SM).
+// One column segment of the y-sweep (rows c0 .. c0+seg-1 of column col); returns whether a cell asked for RK4
+// sub-stepping (SRC_FAST only; the caller then redoes the segment with SRC_EXACT -- the pass is out of place).
+template <int MODE, int SRC>
+__device__ __forceinline__ bool y_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
+                                          int seg, int col, const double* __restrict__ s_tab, double (*s_q)[7][YT], double (*s_w)[9][YT],
+                                          double (*s_r)[YT], double& smax, int& bad)
+{
+    const int tid = threadIdx.x;
+    bool hot = false;
+    const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
+    const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
+    const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
+    const long long fs = P.fstride, pitch = P.pitch;
+    // field order of the sweep: normal momentum = q3, tangential = q2
+    const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
+    double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
+    const int nrows = c1 - c0 + 4;
+    cp_async8(&s_q[0][0][tid], g); cp_async8(&s_q[0][1][tid], g + fs); cp_async8(&s_q[0][2][tid], g + 3 * fs);
+    cp_async8(&s_q[0][3][tid], g + 2 * fs); cp_async8(&s_q[0][4][tid], g + 4 * fs); cp_async8(&s_q[0][5][tid], g + 5 * fs);
+    cp_async8(&s_q[0][6][tid], g + 6 * fs);
+    cp_async_commit();
+    g += pitch;
+    double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
+    int st = 0;                                   // stage of row jj (jj mod 3)
+    for (int jj = 0; jj < nrows; ++jj) {          // row c = c0 - 2 + jj
+        const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
+        if (jj + 1 < nrows) {
+            cp_async8(&s_q[sn][0][tid], g); cp_async8(&s_q[sn][1][tid], g + fs); cp_async8(&s_q[sn][2][tid], g + 3 * fs);
+            cp_async8(&s_q[sn][3][tid], g + 2 * fs); cp_async8(&s_q[sn][4][tid], g + 4 * fs); cp_async8(&s_q[sn][5][tid], g + 5 * fs);
+            cp_async8(&s_q[sn][6][tid], g + 6 * fs);
+            g += pitch;
+        }
+        cp_async_commit();
+        cp_async_wait<1>();
+        FCell Wp;
+        {
+            double q[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) q[k] = s_q[st][k][tid];
+            double dE, q6n;
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n, hot);
+        }
+        // The body is branch free: during the 4 ramp-up rows it runs on not-yet-valid window / face / flux values
+        // (finite or not, never stored: the store and the wavespeed contribution are predicated on jj >= 4).
+        double WL[7], WR[7], lam0c;
+        {                                         // centre cell c-1: s_w[0] = W(c-1), s_w[1][0..6] = W(c-1) - W(c-2)
+            FCell W0;
+            W0.r1 = s_w[0][0][tid]; W0.r2 = s_w[0][1][tid]; W0.un = s_w[0][2][tid]; W0.ut = s_w[0][3][tid]; W0.p = s_w[0][4][tid];
+            W0.z1 = s_w[0][5][tid]; W0.lam = s_w[0][6][tid]; W0.irho = s_w[0][7][tid]; W0.rc2 = s_w[0][8][tid];
+            double a[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) a[k] = s_w[1][k][tid];
+            const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
+            lam0c = W0.lam;
+            recon_core(P, W0, a, b, khalf, WL, WR);
+#pragma unroll
+            for (int k = 0; k < 7; ++k) s_w[1][k][tid] = b[k];
+        }
+        s_w[0][0][tid] = Wp.r1; s_w[0][1][tid] = Wp.r2; s_w[0][2][tid] = Wp.un; s_w[0][3][tid] = Wp.ut; s_w[0][4][tid] = Wp.p;
+        s_w[0][5][tid] = Wp.z1; s_w[0][6][tid] = Wp.lam; s_w[0][7][tid] = Wp.irho; s_w[0][8][tid] = Wp.rc2;
+        FFace fl, fr, pr;
+        face_fast(P, s_tab, WL, fl);
+        face_fast(P, s_tab, WR, fr);
+        pr.r1 = s_r[0][tid]; pr.r2 = s_r[1][tid]; pr.un = s_r[2][tid]; pr.ut = s_r[3][tid]; pr.p = s_r[4][tid];
+        pr.z1 = s_r[5][tid]; pr.lam = s_r[6][tid]; pr.rho = s_r[7][tid]; pr.rhoE = s_r[8][tid]; pr.c = s_r[9][tid];
+        s_r[0][tid] = fr.r1; s_r[1][tid] = fr.r2; s_r[2][tid] = fr.un; s_r[3][tid] = fr.ut; s_r[4][tid] = fr.p;
+        s_r[5][tid] = fr.z1; s_r[6][tid] = fr.lam; s_r[7][tid] = fr.rho; s_r[8][tid] = fr.rhoE; s_r[9][tid] = fr.c;
+        double F[8];
+        hllc_fast(pr, fl, F);                     // face between cells c-2 and c-1
+        {                                         // finish cell c-2
+            double o[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
+            o[5] = fma(dtdx * z1n, F[7], o[5]);                           // R8: non-conservative z1 term
+            o[5] = clampf(o[5], P.z_min, P.z_max);
+            const bool valid = jj >= 4;
+            if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
+                double sm1 = 0.0; int bad1 = 0; bool hot1 = false;
+                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE>(P, s_tab, o, tau, Tsafe, sm1, bad1, hot1);
+                smax = valid ? dmax_(smax, sm1) : smax;
+                bad |= valid ? bad1 : 0;
+                hot |= valid && hot1;
+            }
+            if (valid) {
+                pout[0] = o[0]; pout[fs] = o[1]; pout[3 * fs] = o[2]; pout[2 * fs] = o[3]; pout[4 * fs] = o[4]; pout[5 * fs] = o[5];
+                pout[6 * fs] = o[6];
+                pout += pitch;
+            }
+        }
+        {                                         // start cell c-1 with its lower-face flux
+            double o[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) o[k] = s_q[sp][k][tid];
+            if (MODE == MODE_LEAD) lead_fix(P, o, lam0c);
+            z1n = o[5];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) acc[k] = fma(dtdx, F[k], o[k]);
+            acc[5] = fma(-dtdx * z1n, F[7], acc[5]);
+        }
+        st = sn;
+    }
+    cp_async_wait<0>();
+    return hot;
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin,
                                                                   double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg)
@@ -337,257 +448,188 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
     double (*s_r)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + (YST * 7 + 9 + 7) * YT);
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
-    const int tid = threadIdx.x;
-    const int col = blockIdx.x * YT + tid;
+    const int col = blockIdx.x * YT + threadIdx.x;
+    constexpr bool HAS_SRC = MODE == MODE_LEAD || MODE == MODE_TRAIL;
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
-        const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
-        const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
-        const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
-        const long long fs = P.fstride, pitch = P.pitch;
-        // field order of the sweep: normal momentum = q3, tangential = q2
-        const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
-        double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
-        const int nrows = c1 - c0 + 4;
-        cp_async8(&s_q[0][0][tid], g); cp_async8(&s_q[0][1][tid], g + fs); cp_async8(&s_q[0][2][tid], g + 3 * fs);
-        cp_async8(&s_q[0][3][tid], g + 2 * fs); cp_async8(&s_q[0][4][tid], g + 4 * fs); cp_async8(&s_q[0][5][tid], g + 5 * fs);
-        cp_async8(&s_q[0][6][tid], g + 6 * fs);
-        cp_async_commit();
-        g += pitch;
-        double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
-        int st = 0;                                   // stage of row jj (jj mod 3)
-        for (int jj = 0; jj < nrows; ++jj) {          // row c = c0 - 2 + jj
-            const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
-            if (jj + 1 < nrows) {
-                cp_async8(&s_q[sn][0][tid], g); cp_async8(&s_q[sn][1][tid], g + fs); cp_async8(&s_q[sn][2][tid], g + 3 * fs);
-                cp_async8(&s_q[sn][3][tid], g + 2 * fs); cp_async8(&s_q[sn][4][tid], g + 4 * fs); cp_async8(&s_q[sn][5][tid], g + 5 * fs);
-                cp_async8(&s_q[sn][6][tid], g + 6 * fs);
-                g += pitch;
-            }
-            cp_async_commit();
-            cp_async_wait<1>();
-            FCell Wp;
-            {
-                double q[7];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) q[k] = s_q[st][k][tid];
-                double dE, q6n;
-                prim_cell<MODE == MODE_LEAD>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n);
-            }
-            // The body is branch free: during the 4 ramp-up rows it runs on not-yet-valid window / face / flux values
-            // (finite or not, never stored: the store and the wavespeed contribution are predicated on jj >= 4).
-            double WL[7], WR[7], lam0c;
-            {                                         // centre cell c-1: s_w[0] = W(c-1), s_w[1][0..6] = W(c-1) - W(c-2)
-                FCell W0;
-                W0.r1 = s_w[0][0][tid]; W0.r2 = s_w[0][1][tid]; W0.un = s_w[0][2][tid]; W0.ut = s_w[0][3][tid]; W0.p = s_w[0][4][tid];
-                W0.z1 = s_w[0][5][tid]; W0.lam = s_w[0][6][tid]; W0.irho = s_w[0][7][tid]; W0.rc2 = s_w[0][8][tid];
-                double a[7];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) a[k] = s_w[1][k][tid];
-                const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
-                lam0c = W0.lam;
-                recon_core(P, W0, a, b, khalf, WL, WR);
-#pragma unroll
-                for (int k = 0; k < 7; ++k) s_w[1][k][tid] = b[k];
-            }
-            s_w[0][0][tid] = Wp.r1; s_w[0][1][tid] = Wp.r2; s_w[0][2][tid] = Wp.un; s_w[0][3][tid] = Wp.ut; s_w[0][4][tid] = Wp.p;
-            s_w[0][5][tid] = Wp.z1; s_w[0][6][tid] = Wp.lam; s_w[0][7][tid] = Wp.irho; s_w[0][8][tid] = Wp.rc2;
-            FFace fl, fr, pr;
-            face_fast(P, s_tab, WL, fl);
-            face_fast(P, s_tab, WR, fr);
-            pr.r1 = s_r[0][tid]; pr.r2 = s_r[1][tid]; pr.un = s_r[2][tid]; pr.ut = s_r[3][tid]; pr.p = s_r[4][tid];
-            pr.z1 = s_r[5][tid]; pr.lam = s_r[6][tid]; pr.rho = s_r[7][tid]; pr.rhoE = s_r[8][tid]; pr.c = s_r[9][tid];
-            s_r[0][tid] = fr.r1; s_r[1][tid] = fr.r2; s_r[2][tid] = fr.un; s_r[3][tid] = fr.ut; s_r[4][tid] = fr.p;
-            s_r[5][tid] = fr.z1; s_r[6][tid] = fr.lam; s_r[7][tid] = fr.rho; s_r[8][tid] = fr.rhoE; s_r[9][tid] = fr.c;
-            double F[8];
-            hllc_fast(pr, fl, F);                     // face between cells c-2 and c-1
-            {                                         // finish cell c-2
-                double o[7];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
-                o[5] = fma(dtdx * z1n, F[7], o[5]);                           // R8: non-conservative z1 term
-                o[5] = clampf(o[5], P.z_min, P.z_max);
-                const bool valid = jj >= 4;
-                if (MODE == MODE_TRAIL) {
-                    double sm1 = 0.0; int bad1 = 0;
-                    trail_cell(P, s_tab, o, tau, Tsafe, sm1, bad1);
-                    smax = valid ? dmax_(smax, sm1) : smax;
-                    bad |= valid ? bad1 : 0;
-                }
-                if (valid) {
-                    pout[0] = o[0]; pout[fs] = o[1]; pout[3 * fs] = o[2]; pout[2 * fs] = o[3]; pout[4 * fs] = o[4]; pout[5 * fs] = o[5];
-                    pout[6 * fs] = o[6];
-                    pout += pitch;
-                }
-            }
-            {                                         // start cell c-1 with its lower-face flux
-                double o[7];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) o[k] = s_q[sp][k][tid];
-                if (MODE == MODE_LEAD) lead_fix(P, o, lam0c);
-                z1n = o[5];
-#pragma unroll
-                for (int k = 0; k < 7; ++k) acc[k] = fma(dtdx, F[k], o[k]);
-                acc[5] = fma(-dtdx * z1n, F[7], acc[5]);
-            }
-            st = sn;
+        const bool hot = y_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+        if (HAS_SRC && __any_sync(__activemask(), hot)) {        // rare: redo the warp's segment with the exact R13 rule
+            smax = 0.0; bad = 0;
+            y_segment<MODE, SRC_EXACT>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
         }
-        cp_async_wait<0>();
     }
-    if (MODE == MODE_TRAIL) reduce_smax(smax, bad, ctl);
+    if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // x-sweep (a4): warp per row segment, 2 cells per lane, shared-memory rings between lanes
 // ---------------------------------------------------------------------------------------------------------------
+// One row segment of the x-sweep (cells c0 .. c0+seg-1 of row `row`, one warp); returns whether a cell asked for RK4
+// sub-stepping (SRC_FAST only; the caller then redoes the segment with SRC_EXACT -- the pass is out of place).
+template <int MODE, int SRC>
+__device__ __forceinline__ bool x_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
+                                          int seg, int row, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* s_ring = s_dyn;
+    bool hot = false;
+    double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
+    double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
+    double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
+    double2* stg = reinterpret_cast<double2*>(s_dyn + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
+    const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
+    const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
+    const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
+    const long long fs = P.fstride;
+    const double* rin = qin + (long long)(row + NGY) * P.pitch + NGX;
+    double* rout = qout + (long long)(row + NGY) * P.pitch + NGX;
+    const int nxe = (P.nx + 1) & ~1;                 // last pair base that is ever needed (cell nx+1 is the outer ghost; for odd nx the pair ends in row padding)
+    const int niter = (c1 - c0 + 63) >> 6;
+    const bool fixed_in = (MODE == MODE_LEAD) && (P.bc_xlo == 3);
+    int sw = lane;                                   // ring slot written by this lane: (32 k + lane) mod 33
+    int ps = lane;                                   // staging slot of this lane's pair: (32 k + lane) mod 66
+    {   // stage chunk 0 (cells c0-62 .. c0+1; only lanes 30, 31 are used)
+        const int Ac = min(max(c0 - 64 + 2 * lane + 2, -2), nxe);
+#pragma unroll
+        for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + ps), rin + Ac + f * fs);
+        cp_async_commit();
+    }
+    for (int k = 0; k <= niter; ++k) {
+        const int b = c0 + 64 * (k - 1);             // first cell updated in this iteration
+        const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
+        // iteration 0 only primes the rings (cells c0-2 .. c0+1 through lanes 30, 31); the body is branch free and
+        // simply runs on clamped / not-yet-valid data there, nothing of which is stored
+        const int sr = sw == 0 ? RING - 1 : sw - 1;  // left neighbour's slot
+        FCell WA, WB;
+        const int psn = ps + 32 >= PRING ? ps + 32 - PRING : ps + 32;
+        if (k < niter) {                             // stage the next chunk while this one is computed
+            const int An = min(A + 64, nxe);
+#pragma unroll
+            for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + psn), rin + An + f * fs);
+        }
+        cp_async_commit();
+        cp_async_wait<1>();
+        // ---- phase 1: primitives (+ leading source) of the staged pair -----------------------------------------
+        {
+            const int Ac = min(max(A, -2), nxe);
+            double qa[7], qb[7];
+#pragma unroll
+            for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
+            double dE, q6n;
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n, hot);
+            rw[0 * RING + sw] = WA.r1; rw[1 * RING + sw] = WA.r2; rw[2 * RING + sw] = WA.un; rw[3 * RING + sw] = WA.ut;
+            rw[4 * RING + sw] = WA.p;  rw[5 * RING + sw] = WA.z1; rw[6 * RING + sw] = WA.lam;
+            rw[7 * RING + sw] = WB.r1; rw[8 * RING + sw] = WB.r2; rw[9 * RING + sw] = WB.un; rw[10 * RING + sw] = WB.ut;
+            rw[11 * RING + sw] = WB.p; rw[12 * RING + sw] = WB.z1; rw[13 * RING + sw] = WB.lam;
+            rw[14 * RING + sw] = WB.irho; rw[15 * RING + sw] = WB.rc2;
+        }
+        __syncwarp();
+        // ---- phase 2: reconstruct cells A-1 and A, four face states ------------------------------------------
+        FFace FL1, FR1, FL2;
+        double lam_u0 = 0.0, lam_u1 = 0.0;
+        {
+            FCell Wmm, Wm1;
+            Wmm.r1 = rw[0 * RING + sr]; Wmm.r2 = rw[1 * RING + sr]; Wmm.un = rw[2 * RING + sr]; Wmm.ut = rw[3 * RING + sr];
+            Wmm.p = rw[4 * RING + sr];  Wmm.z1 = rw[5 * RING + sr]; Wmm.lam = rw[6 * RING + sr]; Wmm.irho = 0.0; Wmm.rc2 = 0.0;
+            Wm1.r1 = rw[7 * RING + sr]; Wm1.r2 = rw[8 * RING + sr]; Wm1.un = rw[9 * RING + sr]; Wm1.ut = rw[10 * RING + sr];
+            Wm1.p = rw[11 * RING + sr]; Wm1.z1 = rw[12 * RING + sr]; Wm1.lam = rw[13 * RING + sr];
+            Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
+            lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
+            double WL[7], WR[7];
+            recon_fast(P, Wmm, Wm1, WA, khalf, WL, WR);
+            face_fast(P, s_tab, WL, FL1);
+            face_fast(P, s_tab, WR, FR1);
+            recon_fast(P, Wm1, WA, WB, khalf, WL, WR);
+            face_fast(P, s_tab, WL, FL2);
+            FFace FR2;
+            face_fast(P, s_tab, WR, FR2);
+            rfr[0 * RING + sw] = FR2.r1; rfr[1 * RING + sw] = FR2.r2; rfr[2 * RING + sw] = FR2.un; rfr[3 * RING + sw] = FR2.ut;
+            rfr[4 * RING + sw] = FR2.p;  rfr[5 * RING + sw] = FR2.z1; rfr[6 * RING + sw] = FR2.lam; rfr[7 * RING + sw] = FR2.rho;
+            rfr[8 * RING + sw] = FR2.rhoE; rfr[9 * RING + sw] = FR2.c;
+        }
+        __syncwarp();
+        // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
+        double F1[8], F2[8];
+        {
+            FFace FRp;
+            FRp.r1 = rfr[0 * RING + sr]; FRp.r2 = rfr[1 * RING + sr]; FRp.un = rfr[2 * RING + sr]; FRp.ut = rfr[3 * RING + sr];
+            FRp.p = rfr[4 * RING + sr];  FRp.z1 = rfr[5 * RING + sr]; FRp.lam = rfr[6 * RING + sr]; FRp.rho = rfr[7 * RING + sr];
+            FRp.rhoE = rfr[8 * RING + sr]; FRp.c = rfr[9 * RING + sr];
+            hllc_fast(FRp, FL1, F1);
+            hllc_fast(FR1, FL2, F2);
+#pragma unroll
+            for (int f = 0; f < 8; ++f) rf[f * RING + sw] = F2[f];
+        }
+        __syncwarp();
+        // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
+        const int u0 = b + 2 * lane;
+        {
+            const bool valid = k > 0 && u0 < c1;
+            double F0[8];
+#pragma unroll
+            for (int f = 0; f < 8; ++f) F0[f] = rf[f * RING + sr];
+            const int pl = ps == 0 ? PRING - 1 : ps - 1;      // the pair staged by the left neighbour = cells u0, u0+1
+            double oa[7], ob[7];
+#pragma unroll
+            for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + pl]; oa[f] = v.x; ob[f] = v.y; }
+            if (MODE == MODE_LEAD) {
+                lead_fix(P, oa, lam_u0);
+                lead_fix(P, ob, lam_u1);
+            }
+            const double za = oa[5], zb = ob[5];
+#pragma unroll
+            for (int f = 0; f < 7; ++f) { oa[f] = fma(-dtdx, F1[f] - F0[f], oa[f]); ob[f] = fma(-dtdx, F2[f] - F1[f], ob[f]); }
+            oa[5] = clampf(fma(dtdx * za, F1[7] - F0[7], oa[5]), P.z_min, P.z_max);       // R8
+            ob[5] = clampf(fma(dtdx * zb, F2[7] - F1[7], ob[5]), P.z_min, P.z_max);
+            const bool two = u0 + 1 < c1;
+            if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
+                double sm1 = 0.0, sm2 = 0.0; int bad1 = 0, bad2 = 0; bool hot1 = false, hot2 = false;
+                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE>(P, s_tab, oa, tau, Tsafe, sm1, bad1, hot1);
+                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE>(P, s_tab, ob, tau, Tsafe, sm2, bad2, hot2);
+                sm1 = valid ? sm1 : 0.0; sm2 = (valid && two) ? sm2 : 0.0;
+                smax = dmax_(smax, dmax_(sm1, sm2));
+                bad |= (valid ? bad1 : 0) | ((valid && two) ? bad2 : 0);
+                hot |= (valid && hot1) || (valid && two && hot2);
+            }
+            double* po = rout + u0;
+            if (valid) {
+                if (two) {
+#pragma unroll
+                    for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
+                } else {
+#pragma unroll
+                    for (int f = 0; f < 7; ++f) po[f * fs] = oa[f];
+                }
+            }
+        }
+        sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
+        ps = psn;
+    }
+    cp_async_wait<0>();
+    return hot;
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
                                                     const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
     extern __shared__ __align__(16) double s_dyn[];
     __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
-    double* s_ring = s_dyn;
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int row = blockIdx.x * XW + warp;
+    const int row = blockIdx.x * XW + (threadIdx.x >> 5);
+    constexpr bool HAS_SRC = MODE == MODE_LEAD || MODE == MODE_TRAIL;
     double smax = 0.0; int bad = 0;
     if (row < P.ny) {
-        double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
-        double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
-        double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
-        double2* stg = reinterpret_cast<double2*>(s_dyn + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
-        const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
-        const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
-        const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
-        const long long fs = P.fstride;
-        const double* rin = qin + (long long)(row + NGY) * P.pitch + NGX;
-        double* rout = qout + (long long)(row + NGY) * P.pitch + NGX;
-        const int nxe = (P.nx + 1) & ~1;                 // last pair base that is ever needed (cell nx+1 is the outer ghost; for odd nx the pair ends in row padding)
-        const int niter = (c1 - c0 + 63) >> 6;
-        const bool fixed_in = (MODE == MODE_LEAD) && (P.bc_xlo == 3);
-        int sw = lane;                                   // ring slot written by this lane: (32 k + lane) mod 33
-        int ps = lane;                                   // staging slot of this lane's pair: (32 k + lane) mod 66
-        {   // stage chunk 0 (cells c0-62 .. c0+1; only lanes 30, 31 are used)
-            const int Ac = min(max(c0 - 64 + 2 * lane + 2, -2), nxe);
-#pragma unroll
-            for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + ps), rin + Ac + f * fs);
-            cp_async_commit();
+        const bool hot = x_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
+        if (HAS_SRC && __any_sync(0xffffffffu, hot)) {           // rare: redo the warp's segment with the exact R13 rule
+            smax = 0.0; bad = 0;
+            __syncwarp();
+            x_segment<MODE, SRC_EXACT>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
         }
-        for (int k = 0; k <= niter; ++k) {
-            const int b = c0 + 64 * (k - 1);             // first cell updated in this iteration
-            const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
-            // iteration 0 only primes the rings (cells c0-2 .. c0+1 through lanes 30, 31); the body is branch free and
-            // simply runs on clamped / not-yet-valid data there, nothing of which is stored
-            const int sr = sw == 0 ? RING - 1 : sw - 1;  // left neighbour's slot
-            FCell WA, WB;
-            const int psn = ps + 32 >= PRING ? ps + 32 - PRING : ps + 32;
-            if (k < niter) {                             // stage the next chunk while this one is computed
-                const int An = min(A + 64, nxe);
-#pragma unroll
-                for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + psn), rin + An + f * fs);
-            }
-            cp_async_commit();
-            cp_async_wait<1>();
-            // ---- phase 1: primitives (+ leading source) of the staged pair -----------------------------------------
-            {
-                const int Ac = min(max(A, -2), nxe);
-                double qa[7], qb[7];
-#pragma unroll
-                for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
-                double dE, q6n;
-                prim_cell<MODE == MODE_LEAD>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n);
-                prim_cell<MODE == MODE_LEAD>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n);
-                rw[0 * RING + sw] = WA.r1; rw[1 * RING + sw] = WA.r2; rw[2 * RING + sw] = WA.un; rw[3 * RING + sw] = WA.ut;
-                rw[4 * RING + sw] = WA.p;  rw[5 * RING + sw] = WA.z1; rw[6 * RING + sw] = WA.lam;
-                rw[7 * RING + sw] = WB.r1; rw[8 * RING + sw] = WB.r2; rw[9 * RING + sw] = WB.un; rw[10 * RING + sw] = WB.ut;
-                rw[11 * RING + sw] = WB.p; rw[12 * RING + sw] = WB.z1; rw[13 * RING + sw] = WB.lam;
-                rw[14 * RING + sw] = WB.irho; rw[15 * RING + sw] = WB.rc2;
-            }
-            __syncwarp();
-            // ---- phase 2: reconstruct cells A-1 and A, four face states ------------------------------------------
-            FFace FL1, FR1, FL2;
-            double lam_u0 = 0.0, lam_u1 = 0.0;
-            {
-                FCell Wmm, Wm1;
-                Wmm.r1 = rw[0 * RING + sr]; Wmm.r2 = rw[1 * RING + sr]; Wmm.un = rw[2 * RING + sr]; Wmm.ut = rw[3 * RING + sr];
-                Wmm.p = rw[4 * RING + sr];  Wmm.z1 = rw[5 * RING + sr]; Wmm.lam = rw[6 * RING + sr]; Wmm.irho = 0.0; Wmm.rc2 = 0.0;
-                Wm1.r1 = rw[7 * RING + sr]; Wm1.r2 = rw[8 * RING + sr]; Wm1.un = rw[9 * RING + sr]; Wm1.ut = rw[10 * RING + sr];
-                Wm1.p = rw[11 * RING + sr]; Wm1.z1 = rw[12 * RING + sr]; Wm1.lam = rw[13 * RING + sr];
-                Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
-                lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
-                double WL[7], WR[7];
-                recon_fast(P, Wmm, Wm1, WA, khalf, WL, WR);
-                face_fast(P, s_tab, WL, FL1);
-                face_fast(P, s_tab, WR, FR1);
-                recon_fast(P, Wm1, WA, WB, khalf, WL, WR);
-                face_fast(P, s_tab, WL, FL2);
-                FFace FR2;
-                face_fast(P, s_tab, WR, FR2);
-                rfr[0 * RING + sw] = FR2.r1; rfr[1 * RING + sw] = FR2.r2; rfr[2 * RING + sw] = FR2.un; rfr[3 * RING + sw] = FR2.ut;
-                rfr[4 * RING + sw] = FR2.p;  rfr[5 * RING + sw] = FR2.z1; rfr[6 * RING + sw] = FR2.lam; rfr[7 * RING + sw] = FR2.rho;
-                rfr[8 * RING + sw] = FR2.rhoE; rfr[9 * RING + sw] = FR2.c;
-            }
-            __syncwarp();
-            // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
-            double F1[8], F2[8];
-            {
-                FFace FRp;
-                FRp.r1 = rfr[0 * RING + sr]; FRp.r2 = rfr[1 * RING + sr]; FRp.un = rfr[2 * RING + sr]; FRp.ut = rfr[3 * RING + sr];
-                FRp.p = rfr[4 * RING + sr];  FRp.z1 = rfr[5 * RING + sr]; FRp.lam = rfr[6 * RING + sr]; FRp.rho = rfr[7 * RING + sr];
-                FRp.rhoE = rfr[8 * RING + sr]; FRp.c = rfr[9 * RING + sr];
-                hllc_fast(FRp, FL1, F1);
-                hllc_fast(FR1, FL2, F2);
-#pragma unroll
-                for (int f = 0; f < 8; ++f) rf[f * RING + sw] = F2[f];
-            }
-            __syncwarp();
-            // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
-            const int u0 = b + 2 * lane;
-            {
-                const bool valid = k > 0 && u0 < c1;
-                double F0[8];
-#pragma unroll
-                for (int f = 0; f < 8; ++f) F0[f] = rf[f * RING + sr];
-                const int pl = ps == 0 ? PRING - 1 : ps - 1;      // the pair staged by the left neighbour = cells u0, u0+1
-                double oa[7], ob[7];
-#pragma unroll
-                for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + pl]; oa[f] = v.x; ob[f] = v.y; }
-                if (MODE == MODE_LEAD) {
-                    lead_fix(P, oa, lam_u0);
-                    lead_fix(P, ob, lam_u1);
-                }
-                const double za = oa[5], zb = ob[5];
-#pragma unroll
-                for (int f = 0; f < 7; ++f) { oa[f] = fma(-dtdx, F1[f] - F0[f], oa[f]); ob[f] = fma(-dtdx, F2[f] - F1[f], ob[f]); }
-                oa[5] = clampf(fma(dtdx * za, F1[7] - F0[7], oa[5]), P.z_min, P.z_max);       // R8
-                ob[5] = clampf(fma(dtdx * zb, F2[7] - F1[7], ob[5]), P.z_min, P.z_max);
-                const bool two = u0 + 1 < c1;
-                if (MODE == MODE_TRAIL) {
-                    double sm1 = 0.0, sm2 = 0.0; int bad1 = 0, bad2 = 0;
-                    trail_cell(P, s_tab, oa, tau, Tsafe, sm1, bad1);
-                    trail_cell(P, s_tab, ob, tau, Tsafe, sm2, bad2);
-                    sm1 = valid ? sm1 : 0.0; sm2 = (valid && two) ? sm2 : 0.0;
-                    smax = dmax_(smax, dmax_(sm1, sm2));
-                    bad |= (valid ? bad1 : 0) | ((valid && two) ? bad2 : 0);
-                }
-                double* po = rout + u0;
-                if (valid) {
-                    if (two) {
-#pragma unroll
-                        for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
-                    } else {
-#pragma unroll
-                        for (int f = 0; f < 7; ++f) po[f * fs] = oa[f];
-                    }
-                }
-            }
-            sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
-            ps = psn;
-        }
-        cp_async_wait<0>();
     }
-    if (MODE == MODE_TRAIL) reduce_smax(smax, bad, ctl);
+    if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -605,8 +647,8 @@ __global__ void __launch_bounds__(128) k_source_fast(const __grid_constant__ Par
     double c[7];
 #pragma unroll
     for (int k = 0; k < 7; ++k) c[k] = q[k * P.fstride + id];
-    FCell W; double dE, q6n;
-    prim_cell<true>(P, s_tab, c, dtp[0], dtp[1], W, dE, q6n);
+    FCell W; double dE, q6n; bool hot = false;
+    prim_cell<SRC_EXACT>(P, s_tab, c, dtp[0], dtp[1], W, dE, q6n, hot);
     q[4 * P.fstride + id] = c[4] + dE;
     q[6 * P.fstride + id] = q6n;
 }
@@ -680,13 +722,18 @@ void init_fused_kernels()
     cudaFuncSetAttribute(k_xsweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
     cudaFuncSetAttribute(k_xsweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
     cudaFuncSetAttribute(k_xsweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
+    cudaFuncSetAttribute(k_xsweep<MODE_TRAIL_INERT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
     cudaFuncSetAttribute(k_ysweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
     cudaFuncSetAttribute(k_ysweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
     cudaFuncSetAttribute(k_ysweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
+    cudaFuncSetAttribute(k_ysweep<MODE_TRAIL_INERT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
 }
 
+// mode 0 plain, 1 leading source on load, 2 trailing source + max-wavespeed partial.  An inert run (P.reactive = 0) has
+// no source step: its pass 1 is the plain sweep and its pass 2 the sweep + wavespeed.
 void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s)
 {
+    if (!P.reactive) mode = mode == MODE_LEAD ? MODE_PLAIN : (mode == MODE_TRAIL ? MODE_TRAIL_INERT : mode);
     if (dir == 0) {
         const int lines = (P.ny + XW - 1) / XW;
         const int seg = pick_seg(P.nx, 64, 2048, 64, lines, num_sms() * NMSDT_X_MINBLOCKS);
@@ -694,7 +741,8 @@ void launch_sweep_fused(const Params& P, const double* qin, double* qout, const 
         const size_t sm = XS_DOUBLES * sizeof(double);
         if (mode == MODE_PLAIN)      k_xsweep<MODE_PLAIN><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
         else if (mode == MODE_LEAD)  k_xsweep<MODE_LEAD><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_xsweep<MODE_TRAIL><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_TRAIL) k_xsweep<MODE_TRAIL><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_xsweep<MODE_TRAIL_INERT><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
         const int seg = pick_seg(P.ny, 1, 128, 4, lines, num_sms() * NMSDT_Y_MINBLOCKS);
@@ -702,7 +750,8 @@ void launch_sweep_fused(const Params& P, const double* qin, double* qout, const 
         const size_t sm = YS_DOUBLES * sizeof(double);
         if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
         else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_ysweep<MODE_TRAIL><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else if (mode == MODE_TRAIL) k_ysweep<MODE_TRAIL><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        else                         k_ysweep<MODE_TRAIL_INERT><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
     }
 }
 

@@ -225,6 +225,51 @@ def test_one_step_parity(O, B, name, kw, pre, variant):
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
+def test_rare_paths_substepped_source_inside_full_steps(O, B, variant):
+    """R13 inside sim_step: with theta_0 lowered to 2e-5 every shocked cell needs several RK4 sub-steps, so the fused
+    kernels take their redo path (a warp whose segment holds such a cell repeats it with the exact rule)."""
+    cfg = inputs.config("C1", reactive=1)
+    o0 = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=8)
+    o0.init(cfg["init"])
+    o0.step(400)
+    cfg["kin"]["substep_theta"] = 2e-5
+    o, s = _pair(O, B, cfg, variant=variant)
+    o.init_fields(o0.state())
+    _sync_state(o, s)
+    e = O.make_eos(cfg["eos"]); k = O.make_kin(cfg["kin"])
+    q = np.array([f[64, 20] for f in o.state()])                 # a cell of the shocked slab's wake
+    assert O.source_cell(e, k, q, 0.5 * o.cfl_dt())[1] > 1       # the rule really asks for sub-steps there
+    for it in range(2):
+        o.step(1)
+        s.step(1)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="substepped step %d" % it)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("d", [0, 1])
+def test_rare_paths_first_order_fallback(O, B, d, variant):
+    """R17: the scheme never needs the fallback at CFL 0.4 (nor at 10x that step); a sweep with 40x (x) / 160x (y) the
+    CFL step on a developed cavity collapse predicts non-positive face densities in some cells, and both sides must
+    fall back to first order in exactly those cells.  The input state is valid, so every output is finite."""
+    cfg, o = _developed_c1(O, reactive=0, steps=600)
+    s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=variant)
+    _sync_state(o, s)
+    mult = 40.0 if d == 0 else 160.0
+    dt = mult * o.cfl_dt()
+    n0 = o.fallback_count()
+    c_before = o.read_field("c")
+    o.sweep(d, dt)
+    s.sweep(d, dt)
+    assert o.fallback_count() > n0, "the case must trigger the fallback"
+    qa, qb = s.state(), o.state()
+    assert all(np.isfinite(a).all() for a in qa) and all(np.isfinite(b).all() for b in qb)
+    r = rel_diff(qa, qb, c_before)                                # sound speed of the (valid) input state as the momentum scale
+    # the update is q - (dt/dx) dF: the rounding differences of the fluxes are amplified by the step multiplier (a
+    # cell that fell back on one side only would differ by ~1e-2)
+    assert max(r) <= mult * TOL_ONE_STEP, r
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_500_steps_l1_parity_c1(O, B, variant):
     cfg = inputs.config("C1", reactive=1)
     o, s = _pair(O, B, cfg, variant=variant)
