@@ -158,9 +158,10 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     f.c = q_sqrt(floor1(rc2 * q_rcp(xi * rho)));
 }
 
-__device__ __forceinline__ double limited_f(int kind, double a, double b)
+template <int LIM>
+__device__ __forceinline__ double limited_f(double a, double b)
 {
-    if (kind == 0) {                                                              // minmod (R5)
+    if (LIM == 0) {                                                               // minmod (R5)
         // a b > 0 <=> equal sign bits and both non-zero; if either is zero the smaller magnitude is that zero
         const double m = fabs(a) < fabs(b) ? a : b;
         return ((__double2hiint(a) ^ __double2hiint(b)) >= 0) ? m : 0.0;
@@ -174,13 +175,14 @@ __device__ __forceinline__ double limited_f(int kind, double a, double b)
 // R17 first-order fallback (a predicted face density <= 0 -> WL = WR = W0) without a branch: the four densities are
 // predicted first; if one of them is not positive they are replaced by the cell values and the other five slopes are
 // zeroed, which makes their face values equal the cell values exactly (fma(+-0.5, 0, fma(-k, 0, w)) = w).
+template <int LIM>
 __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, const double a[7], const double b[7], double khalf, double WL[7],
                                            double WR[7])
 {
     const double w0[7] = {W0.r1, W0.r2, W0.un, W0.ut, W0.p, W0.z1, W0.lam};
     double D[7];
 #pragma unroll
-    for (int k = 0; k < 7; ++k) D[k] = limited_f(P.limiter, a[k], b[k]);
+    for (int k = 0; k < 7; ++k) D[k] = limited_f<LIM>(a[k], b[k]);
     const double u = W0.un;
     {
         const double m0 = fma(-khalf, fma(u, D[0], W0.r1 * D[2]), w0[0]);
@@ -208,12 +210,13 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
     }
 }
 
+template <int LIM>
 __device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, const FCell& W0, const FCell& Wp, double khalf, double WL[7],
                                            double WR[7])
 {
     const double a[7] = {W0.r1 - Wm.r1, W0.r2 - Wm.r2, W0.un - Wm.un, W0.ut - Wm.ut, W0.p - Wm.p, W0.z1 - Wm.z1, W0.lam - Wm.lam};
     const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
-    recon_core(P, W0, a, b, khalf, WL, WR);
+    recon_core<LIM>(P, W0, a, b, khalf, WL, WR);
 }
 
 // O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
@@ -334,7 +337,7 @@ constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part
 // Only the half-finished update of cell c-1 stays in registers; this keeps the kernel at 128 registers (16 warps/SM).
 // One column segment of the y-sweep (rows c0 .. c0+seg-1 of column col); returns whether a cell asked for RK4
 // sub-stepping (SRC_FAST only; the caller then redoes the segment with SRC_EXACT -- the pass is out of place).
-template <int MODE, int SRC>
+template <int MODE, int SRC, int LIM>
 __device__ __forceinline__ bool y_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
                                           int seg, int col, const double* __restrict__ s_tab, double (*s_q)[7][YT], double (*s_w)[9][YT],
                                           double (*s_r)[YT], double& smax, int& bad)
@@ -386,7 +389,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
             for (int k = 0; k < 7; ++k) a[k] = s_w[1][k][tid];
             const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
             lam0c = W0.lam;
-            recon_core(P, W0, a, b, khalf, WL, WR);
+            recon_core<LIM>(P, W0, a, b, khalf, WL, WR);
 #pragma unroll
             for (int k = 0; k < 7; ++k) s_w[1][k][tid] = b[k];
         }
@@ -437,7 +440,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
     return hot;
 }
 
-template <int MODE>
+template <int MODE, int LIM>
 __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin,
                                                                   double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
@@ -452,10 +455,10 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
     constexpr bool HAS_SRC = MODE == MODE_LEAD || MODE == MODE_TRAIL;
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
-        const bool hot = y_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+        const bool hot = y_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
         if (HAS_SRC && __any_sync(__activemask(), hot)) {        // rare: redo the warp's segment with the exact R13 rule
             smax = 0.0; bad = 0;
-            y_segment<MODE, SRC_EXACT>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+            y_segment<MODE, SRC_EXACT, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
         }
     }
     if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
@@ -466,7 +469,7 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
 // ---------------------------------------------------------------------------------------------------------------
 // One row segment of the x-sweep (cells c0 .. c0+seg-1 of row `row`, one warp); returns whether a cell asked for RK4
 // sub-stepping (SRC_FAST only; the caller then redoes the segment with SRC_EXACT -- the pass is out of place).
-template <int MODE, int SRC>
+template <int MODE, int SRC, int LIM>
 __device__ __forceinline__ bool x_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
                                           int seg, int row, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad)
 {
@@ -537,10 +540,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
             lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
             double WL[7], WR[7];
-            recon_fast(P, Wmm, Wm1, WA, khalf, WL, WR);
+            recon_fast<LIM>(P, Wmm, Wm1, WA, khalf, WL, WR);
             face_fast(P, s_tab, WL, FL1);
             face_fast(P, s_tab, WR, FR1);
-            recon_fast(P, Wm1, WA, WB, khalf, WL, WR);
+            recon_fast<LIM>(P, Wm1, WA, WB, khalf, WL, WR);
             face_fast(P, s_tab, WL, FL2);
             FFace FR2;
             face_fast(P, s_tab, WR, FR2);
@@ -610,7 +613,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
     return hot;
 }
 
-template <int MODE>
+template <int MODE, int LIM>
 __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
                                                     const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
@@ -622,11 +625,11 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
     constexpr bool HAS_SRC = MODE == MODE_LEAD || MODE == MODE_TRAIL;
     double smax = 0.0; int bad = 0;
     if (row < P.ny) {
-        const bool hot = x_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
+        const bool hot = x_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
         if (HAS_SRC && __any_sync(0xffffffffu, hot)) {           // rare: redo the warp's segment with the exact R13 rule
             smax = 0.0; bad = 0;
             __syncwarp();
-            x_segment<MODE, SRC_EXACT>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
+            x_segment<MODE, SRC_EXACT, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
         }
     }
     if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
@@ -715,43 +718,63 @@ static int num_sms()
     return n;
 }
 
+template <int MODE, int LIM>
+static void x_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl,
+                     int seg)
+{
+    if (attr_only) cudaFuncSetAttribute(k_xsweep<MODE, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    else k_xsweep<MODE, LIM><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+}
+template <int MODE, int LIM>
+static void y_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl,
+                     int seg)
+{
+    if (attr_only) cudaFuncSetAttribute(k_ysweep<MODE, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    else k_ysweep<MODE, LIM><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+}
+
+// dispatch on (direction, pass kind, limiter); attr_only = opt in to the dynamic shared memory instead of launching
+static void sweep_dispatch(bool attr_only, int dir, int mode, int lim, dim3 grid, cudaStream_t s, const Params& P, const double* qin, double* qout,
+                           const double* dtp, Ctl* ctl, int seg)
+{
+    const size_t sm = (dir == 0 ? XS_DOUBLES : YS_DOUBLES) * sizeof(double);
+#define NMSDT_CASE(D, M, L)                                                                                          \
+    if (dir == D && mode == M && lim == L) {                                                                        \
+        if (D == 0) x_launch<M, L>(attr_only, grid, sm, s, P, qin, qout, dtp, ctl, seg);                          \
+        else        y_launch<M, L>(attr_only, grid, sm, s, P, qin, qout, dtp, ctl, seg);                          \
+        return;                                                                                                     \
+    }
+    NMSDT_CASE(0, MODE_PLAIN, 0) NMSDT_CASE(0, MODE_LEAD, 0) NMSDT_CASE(0, MODE_TRAIL, 0) NMSDT_CASE(0, MODE_TRAIL_INERT, 0)
+    NMSDT_CASE(0, MODE_PLAIN, 1) NMSDT_CASE(0, MODE_LEAD, 1) NMSDT_CASE(0, MODE_TRAIL, 1) NMSDT_CASE(0, MODE_TRAIL_INERT, 1)
+    NMSDT_CASE(1, MODE_PLAIN, 0) NMSDT_CASE(1, MODE_LEAD, 0) NMSDT_CASE(1, MODE_TRAIL, 0) NMSDT_CASE(1, MODE_TRAIL_INERT, 0)
+    NMSDT_CASE(1, MODE_PLAIN, 1) NMSDT_CASE(1, MODE_LEAD, 1) NMSDT_CASE(1, MODE_TRAIL, 1) NMSDT_CASE(1, MODE_TRAIL_INERT, 1)
+#undef NMSDT_CASE
+}
+
 // opt in to the dynamic shared memory the sweeps need (called once per handle from sim_create, outside any capture)
 void init_fused_kernels()
 {
-    const int smx = (int)(XS_DOUBLES * sizeof(double)), smy = (int)(YS_DOUBLES * sizeof(double));
-    cudaFuncSetAttribute(k_xsweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
-    cudaFuncSetAttribute(k_xsweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
-    cudaFuncSetAttribute(k_xsweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
-    cudaFuncSetAttribute(k_xsweep<MODE_TRAIL_INERT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
-    cudaFuncSetAttribute(k_ysweep<MODE_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
-    cudaFuncSetAttribute(k_ysweep<MODE_LEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
-    cudaFuncSetAttribute(k_ysweep<MODE_TRAIL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
-    cudaFuncSetAttribute(k_ysweep<MODE_TRAIL_INERT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smy);
+    Params P{};
+    for (int dir = 0; dir < 2; ++dir)
+        for (int mode = 0; mode < 4; ++mode)
+            for (int lim = 0; lim < 2; ++lim) sweep_dispatch(true, dir, mode, lim, dim3(1), nullptr, P, nullptr, nullptr, nullptr, nullptr, 0);
 }
 
 // mode 0 plain, 1 leading source on load, 2 trailing source + max-wavespeed partial.  An inert run (P.reactive = 0) has
-// no source step: its pass 1 is the plain sweep and its pass 2 the sweep + wavespeed.
+// no source step: its pass 1 is the plain sweep and its pass 2 the sweep + wavespeed.  The limiter (R5) is a template
+// parameter so that the marching loop stays one basic block.
 void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s)
 {
     if (!P.reactive) mode = mode == MODE_LEAD ? MODE_PLAIN : (mode == MODE_TRAIL ? MODE_TRAIL_INERT : mode);
+    const int lim = P.limiter == 0 ? 0 : 1;
     if (dir == 0) {
         const int lines = (P.ny + XW - 1) / XW;
         const int seg = pick_seg(P.nx, 64, 2048, 64, lines, num_sms() * NMSDT_X_MINBLOCKS);
-        dim3 grid(lines, (P.nx + seg - 1) / seg);
-        const size_t sm = XS_DOUBLES * sizeof(double);
-        if (mode == MODE_PLAIN)      k_xsweep<MODE_PLAIN><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_LEAD)  k_xsweep<MODE_LEAD><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_TRAIL) k_xsweep<MODE_TRAIL><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_xsweep<MODE_TRAIL_INERT><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, P, qin, qout, dtp, ctl, seg);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
         const int seg = pick_seg(P.ny, 1, 128, 4, lines, num_sms() * NMSDT_Y_MINBLOCKS);
-        dim3 grid(lines, (P.ny + seg - 1) / seg);
-        const size_t sm = YS_DOUBLES * sizeof(double);
-        if (mode == MODE_PLAIN)      k_ysweep<MODE_PLAIN><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_LEAD)  k_ysweep<MODE_LEAD><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else if (mode == MODE_TRAIL) k_ysweep<MODE_TRAIL><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
-        else                         k_ysweep<MODE_TRAIL_INERT><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+        sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, P, qin, qout, dtp, ctl, seg);
     }
 }
 

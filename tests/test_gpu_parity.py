@@ -225,6 +225,29 @@ def test_one_step_parity(O, B, name, kw, pre, variant):
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("reactive", [0, 1])
+def test_one_step_parity_mc_limiter(O, B, reactive, variant):
+    """the switchable monotonised-central limiter (R5), reactive and inert (the fused path has kernels of its own for
+    each limiter and for inert runs)"""
+    cfg = inputs.config("C1", reactive=reactive)
+    o0 = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=8)
+    o0.init(cfg["init"])
+    o0.step(400)
+    cfg["grid"]["limiter"] = inputs.LIM_MC
+    o, s = _pair(O, B, cfg, variant=variant)
+    o.init_fields(o0.state())
+    _sync_state(o, s)
+    for it in range(2):
+        o.step(1)
+        s.step(1)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="MC limiter step %d" % it)
+    o_mm = O.Oracle(dict(cfg["grid"], limiter=inputs.LIM_MINMOD), cfg["eos"], cfg["kin"], threads=8)
+    o_mm.init_fields(o0.state())
+    o_mm.step(2)
+    assert max(rel_diff(o_mm.state(), o.state(), o.read_field("c"))) > 1e-6      # the limiter really differs
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_rare_paths_substepped_source_inside_full_steps(O, B, variant):
     """R13 inside sim_step: with theta_0 lowered to 2e-5 every shocked cell needs several RK4 sub-steps, so the fused
     kernels take their redo path (a warp whose segment holds such a cell repeats it with the exact rule)."""
