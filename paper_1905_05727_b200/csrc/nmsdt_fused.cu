@@ -16,7 +16,7 @@
 //             three 33-slot rings in shared memory (slot = lane counter mod 33, so lane 31's entry of the previous
 //             chunk is lane 0's left neighbour: no halo recomputation, no copies); 3 __syncwarp per chunk.
 #include "nmsdt_host.h"
-#include "nmsdt_math.cuh"
+#include "nmsdt_fast.cuh"
 
 namespace nmsdt {
 
@@ -26,118 +26,7 @@ namespace {
 // TRAIL_INERT = sweep + wavespeed (inert runs: pass 1 is PLAIN, pass 2 is TRAIL_INERT)
 enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2, MODE_TRAIL_INERT = 3 };
 
-struct FCell {            // W = (rho1, rho2, un, ut, p, z1, lambda) + what the Hancock predictor needs
-    double r1, r2, un, ut, p, z1, lam;
-    double irho, rc2;     // 1/rho, rho c^2 (with the c >= 1 m/s floor of R10)
-};
 struct FFace { double r1, r2, un, ut, p, z1, lam, rho, rhoE, c; };
-
-__device__ __forceinline__ double clampf(double x, double lo, double hi) { return dmin_(dmax_(x, lo), hi); }
-
-// R13 exact sub-step count (only reached by cells hotter than the safe bound; same exactly-rounded sequence as k_source)
-__device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
-{
-    if (!(Tub > 0.0)) return 1;
-    double y = __ddiv_rn(P.Ta, Tub);
-    double y2 = __dmul_rn(y, y);
-    double den = __dadd_rn(__dadd_rn(__dadd_rn(1.0, y), __ddiv_rn(y2, 2.0)), __ddiv_rn(__dmul_rn(y2, y), 6.0));
-    double g = __ddiv_rn(1.0, den);
-    double theta = __dmul_rn(__dmul_rn(tau, P.Cpre), g);
-    double r = floor(__ddiv_rn(theta, P.theta0));
-    return (r >= (double)(P.max_substeps - 1)) ? P.max_substeps : 1 + (int)r;
-}
-
-// one classic RK4 step of d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)), T2 = T0 + beta (lam0 - lambda), from lam over h
-__device__ __forceinline__ double rk4_step(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double lam,
-                                           double h)
-{
-    const double nTa = P.Ta, mC = -P.Cpre;
-    double l, T, k1, k2, k3, k4;
-    l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = is_pos(T) ? k1 : 0.0;
-    l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = is_pos(T) ? k2 : 0.0;
-    l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = is_pos(T) ? k3 : 0.0;
-    l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = is_pos(T) ? k4 : 0.0;
-    return fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
-}
-
-// R13 sub-stepped integration (only reached by cells hotter than the safe bound)
-__device__ __noinline__ double rk4_substepped(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double tau)
-{
-    const int nsub = nsub_exact(P, fma(beta, lam0, T0), tau);
-    const double h = tau / (double)nsub;
-    double lam = lam0;
-    for (int s = 0; s < nsub; ++s) lam = rk4_step(P, tab, T0, beta, lam0, lam, h);
-    return lam;
-}
-
-// O5: lambda after integrating over tau.
-// SRC_FAST: one RK4 step, straight-line code; `hot` is raised when the temperature bound reaches Tsafe, i.e. when the
-// R13 rule could ask for more than one sub-step: the caller then redoes its whole segment with SRC_EXACT.  Keeping
-// this decision out of the marching loop keeps the loop body one basic block (the serial RK4 chain overlaps with
-// the EOS evaluations of the faces).
-// SRC_EXACT: the R13 rule, sub-stepped integration behind a warp-uniform branch.
-enum { SRC_NONE = 0, SRC_FAST = 1, SRC_EXACT = 2 };
-template <int SRC>
-__device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0,
-                                                double tau, double Tsafe, bool& hot)
-{
-    double lam = rk4_step(P, tab, T0, beta, lam0, lam0, tau);
-    const bool h = fma(beta, lam0, T0) >= Tsafe;
-    if (SRC == SRC_FAST) {
-        hot |= h;
-    } else {
-        if (__any_sync(__activemask(), h)) {
-            const double l2 = rk4_substepped(P, tab, T0, beta, lam0, tau);
-            lam = h ? l2 : lam;
-        }
-    }
-    return dmin_(nonneg(lam), lam0);
-}
-
-// O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.
-// SRC: the Arrhenius step over tau is applied to the cell; dE = energy moved into rho E, q6n = new z2 rho2 lambda.
-// The kernels that apply the source are only launched for reactive runs (launch_sweep_fused), so there is no
-// P.reactive test here.
-template <int SRC>
-__device__ __forceinline__ void prim_cell(const Params& P, const double* __restrict__ tab, const double q[7], double tau, double Tsafe,
-                                          FCell& W, double& dE, double& q6n, bool& hot)
-{
-    const double rho = q[0] + q[1];
-    const double irho = q_rcp(rho);
-    W.irho = irho;
-    W.un = q[2] * irho;
-    W.ut = q[3] * irho;
-    const double z1 = clampf(q[5], P.z_min, P.z_max);
-    const double z2 = 1.0 - z1;
-    const double iq1 = q_rcp(q[1]);
-    W.z1 = z1;
-    W.r1 = q[0] * q_rcp(z1);
-    W.r2 = q[1] * q_rcp(z2);
-    const double rhoe = fma(-0.5 * irho, fma(q[2], q[2], q[3] * q[3]), q[4]);
-    const double x = W.r2 * P.irho02;
-    double xC, xD;
-    q_pow_pair(tab, x, P.C2, P.D2, xC, xD);
-    const double pr = fma(P.A, xC, -P.B * xD);                                   // Eq. 3
-    const double rer = fma(P.kA, xC - x, P.kB * (xD - x));                       // rho2 * Eq. 4
-    const double xi = fma(z1, P.iG1, z2 * P.iG2);
-    const double ixi = q_rcp(xi);
-    double p = (rhoe - z2 * fma(-pr, P.iG2, rer)) * ixi;
-    double lam = clamp01(q[6] * iq1);
-    dE = 0.0; q6n = q[6];
-    if (SRC != SRC_NONE) {
-        const double T0 = P.Tref2 + (p - pr) * (z2 * iq1) * P.iG2cv2;            // Eq. 5 (1/rho2 = z2/q1)
-        const double beta = z2 * P.Q * ixi * P.iG2cv2;
-        const double lam1 = arrhenius_rk4<SRC>(P, tab, T0, beta, lam, tau, Tsafe, hot);
-        dE = q[1] * P.Q * (lam - lam1);
-        q6n = q[1] * lam1;
-        p = fma(dE, ixi, p);                                                     // p is linear in rho e at frozen rho_k, z_k
-        lam = lam1;
-    }
-    W.p = p; W.lam = lam;
-    const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
-    const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22) * ixi;  // R10
-    W.rc2 = dmax_(rc2, rho);                                                      // c^2 >= 1
-}
 
 __device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f)
 {

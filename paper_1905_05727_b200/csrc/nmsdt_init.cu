@@ -1,6 +1,7 @@
 // nmsdt_init.cu -- problem setup (a9: seeded cavity generator, tanh painting, shocked slab),
 // diagnostics reduction (a8; Eq. 12-13) and derived output fields of libnmsdt.so.
 #include "nmsdt_host.h"
+#include "nmsdt_fast.cuh"
 #include <cmath>
 #include <vector>
 
@@ -121,9 +122,12 @@ __device__ __forceinline__ void block_reduce_diag(double v[DIAG_NV], int& bad, d
     }
 }
 
-__global__ void __launch_bounds__(256) k_diag_partial(const __grid_constant__ Params P, const double* __restrict__ q, double* __restrict__ partial)
+__global__ void __launch_bounds__(256, 4) k_diag_partial(const __grid_constant__ Params P, const double* __restrict__ q, double* __restrict__ partial)
 {
     __shared__ double sm[8][DIAG_NV + 1];
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];      // elementary-function tables of nmsdt_math.cuh
+    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
+    __syncthreads();
     double v[DIAG_NV];
 #pragma unroll
     for (int k = 0; k < DIAG_NV; ++k) v[k] = 0.0;
@@ -131,18 +135,23 @@ __global__ void __launch_bounds__(256) k_diag_partial(const __grid_constant__ Pa
     const long long ncell = (long long)P.nx * P.ny;
     const long long per = (ncell + gridDim.x - 1) / gridDim.x;
     const long long a = (long long)blockIdx.x * per, b = min(a + per, ncell);
-    for (long long t = a + threadIdx.x; t < b; t += blockDim.x) {
-        const int j = (int)(t / P.nx), i = (int)(t - (long long)j * P.nx);
+    long long t = a + threadIdx.x;
+    int j = (int)(t / P.nx), i = (int)(t - (long long)j * P.nx);       // one division per thread, then incremental (i, j)
+    for (; t < b; t += blockDim.x, i += blockDim.x) {
+        while (i >= P.nx) { i -= P.nx; ++j; }
         const long long id = (long long)(j + NGY) * P.pitch + NGX + i;
         double c[7];
 #pragma unroll
         for (int k = 0; k < 7; ++k) c[k] = q[k * P.fstride + id];
-        Prim W; double rho, c2, T2;
-        cons_to_prim(P, c, W, rho, c2, &T2);
+        // the pass is bound by HBM only with the fused path's own elementary functions (the CUDA library's log / exp
+        // / sqrt / division make it FP64 bound)
+        FCell W; double dE, q6n; bool hot = false;
+        prim_cell<SRC_NONE>(P, s_tab, c, 0.0, 0.0, W, dE, q6n, hot);
+        const double T2 = cell_T2(P, W);
         v[0] += c[0]; v[1] += c[1]; v[2] += c[2]; v[3] += c[3]; v[4] += c[4]; v[5] += c[6];
-        if (P.reactive && T2 > 0.0) v[6] += c[6] * P.Cpre * exp(-P.Ta / T2);
-        const double sp = fmax(fabs(W.un), fabs(W.ut)) + sqrt(c2);
-        v[7] = fmax(v[7], sp);
+        if (P.reactive && T2 > 0.0) v[6] += c[6] * P.Cpre * q_exp_neg(s_tab, P.Ta * q_rcp(T2));      // Eq. 6 rate
+        const double sp = dmax_(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
+        v[7] = sp > v[7] ? sp : v[7];               // NaN never wins: a bad state is reported through `bad`
         const bool ok = isfinite(c[0]) && isfinite(c[1]) && isfinite(c[2]) && isfinite(c[3]) && isfinite(c[4]) && isfinite(c[5])
                         && isfinite(c[6]) && c[0] > 0.0 && c[1] > 0.0;
         bad |= ok ? 0 : 1;

@@ -5,8 +5,10 @@
 //
 //   k_kinematics                            : moving-averaged shock velocity / acceleration, Eq. C1-C2
 // All sums have a fixed shape (no floating-point atomics): results are bit-identical from run to run.
-// These passes read the state once (56 B/cell) and are bound by HBM; they are not part of sim_step.
+// These passes read the state once (56 B/cell) and are not part of sim_step; with the fused path's own elementary
+// functions (nmsdt_fast.cuh) the primitive recovery is cheap enough for them to be bound by HBM.
 #include "nmsdt_host.h"
+#include "nmsdt_fast.cuh"
 
 namespace nmsdt {
 
@@ -23,6 +25,9 @@ __device__ __forceinline__ void load_cell(const Params& P, const double* __restr
 // partial column sums over the rows of one segment: part[(seg*3 + k)*nx + i], k = 0: p, 1: rho, 2: rho u
 __global__ void __launch_bounds__(PT) k_prof_partial(const __grid_constant__ Params P, const double* __restrict__ q, double* __restrict__ part, int rows_per_seg)
 {
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
+    for (int k = threadIdx.x; k < MATH_TAB_DOUBLES; k += PT) s_tab[k] = P.tab[k];
+    __syncthreads();
     const int i = blockIdx.x * PT + threadIdx.x;
     if (i >= P.nx) return;
     const int j0 = blockIdx.y * rows_per_seg, j1 = min(j0 + rows_per_seg, P.ny);
@@ -30,9 +35,9 @@ __global__ void __launch_bounds__(PT) k_prof_partial(const __grid_constant__ Par
     for (int j = j0; j < j1; ++j) {
         double c[7];
         load_cell(P, q, (long long)(j + NGY) * P.pitch + NGX + i, c);
-        Prim W; double rho, c2;
-        cons_to_prim(P, c, W, rho, c2, nullptr);
-        sp += W.p; sr += rho; sm += c[2];
+        FCell W; double dE, q6n; bool hot = false;
+        prim_cell<SRC_NONE>(P, s_tab, c, 0.0, 0.0, W, dE, q6n, hot);
+        sp += W.p; sr += c[0] + c[1]; sm += c[2];
     }
     double* o = part + (size_t)blockIdx.y * 3 * P.nx + i;
     o[0] = sp; o[P.nx] = sr; o[2 * (size_t)P.nx] = sm;
@@ -75,10 +80,12 @@ constexpr int HT = 256, HW = HT / 32;      // threads / warps per block of the h
 // Eq. 14-16.  Every warp owns whole rows (row = global warp id + k * number of warps) and a private histogram in shared
 // memory; within a 32-cell group the lanes that fall into the same bin are added in lane order by shuffles and the sum
 // is added by one lane, so the order of every floating-point addition is fixed by the launch shape alone.
-__global__ void __launch_bounds__(HT) k_qdot_hist(const __grid_constant__ Params P, const double* __restrict__ q, double n_lo, double dn, int nbins,
+__global__ void __launch_bounds__(HT, 4) k_qdot_hist(const __grid_constant__ Params P, const double* __restrict__ q, double n_lo, double dn, int nbins,
                                                   double* __restrict__ part_mass, unsigned long long* __restrict__ count)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
+    for (int k = threadIdx.x; k < MATH_TAB_DOUBLES; k += HT) s_tab[k] = P.tab[k];
     double* s_mass = reinterpret_cast<double*>(s_raw);                         // [HW][nbins]
     int* s_cnt = reinterpret_cast<int*>(s_raw + (size_t)HW * nbins * sizeof(double));   // [HW][nbins]
     for (int k = threadIdx.x; k < HW * nbins; k += HT) { s_mass[k] = 0.0; s_cnt[k] = 0; }
@@ -97,12 +104,14 @@ __global__ void __launch_bounds__(HT) k_qdot_hist(const __grid_constant__ Params
             if (i < P.nx) {
                 double c[7];
                 load_cell(P, q, row + i, c);
-                Prim W; double rho, c2, T2;
-                cons_to_prim(P, c, W, rho, c2, &T2);
+                FCell W; double dE, q6n; bool hot = false;
+                prim_cell<SRC_NONE>(P, s_tab, c, 0.0, 0.0, W, dE, q6n, hot);
+                const double T2 = cell_T2(P, W);
                 if (T2 > 0.0) {
-                    const double qdot = c[6] * P.Cpre * exp(-P.Ta / T2) * P.Q;          // Eq. 14 [W/m^3]
-                    if (qdot > 0.0) {
-                        const double fb = floor((log10(qdot / 1e9) - n_lo) / dn);       // Eq. 15 [GW/m^3]
+                    const double qdot = c[6] * P.Cpre * q_exp_neg(s_tab, P.Ta * q_rcp(T2)) * P.Q;      // Eq. 14 [W/m^3]
+                    if (qdot > 1e-290) {                                                 // (a flushed exponential is far below any window)
+                        const double n = q_log(s_tab, qdot * 1e-9) * 0.43429448190325182765;          // Eq. 15: log10 of GW/m^3
+                        const double fb = floor((n - n_lo) / dn);
                         if (fb >= 0.0 && fb < (double)nbins) { bin = (int)fb; mass = c[1] * dA; }
                     }
                 }
