@@ -7,7 +7,8 @@ pytestmark = pytest.mark.gpu
 
 
 def test_elementary_functions_device():
-    from paper_1905_05727_b200 import binding, inputs
+    from paper_1905_05727_b200 import binding, build, inputs
+    build.build()
     cfg = inputs.config("C1")
     s = binding.Sim(cfg["grid"], cfg["eos"], cfg["kin"])
     try:
