@@ -31,16 +31,26 @@ __device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
     return (r >= (double)(P.max_substeps - 1)) ? P.max_substeps : 1 + (int)r;
 }
 
+// Arrhenius rate of Eq. 6 at (l, T): -l C exp(-Ta/T) for T > 0, else 0 (O5).  One range test on the high word of
+// y = Ta/T covers both guards: y in [0, 690) <=> T > 0 and exp(-y) above ~1e-300 (the rate is taken as 0 beyond
+// that; 690 = 0x40859000_00000000); T <= 0, T = +0 (y = inf) and NaN all fail the unsigned compare.
+__device__ __forceinline__ double arr_rate(const Params& P, const double* __restrict__ tab, double l, double T)
+{
+    const double y = P.Ta * q_rcp(T);
+    const bool good = (unsigned)hi_word(y) < 0x40859000u;
+    const double k = l * -P.Cpre * q_exp2_prod(tab, y, -KC[9]);
+    return good ? k : 0.0;
+}
+
 // one classic RK4 step of d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)), T2 = T0 + beta (lam0 - lambda), from lam over h
 __device__ __forceinline__ double rk4_step(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double lam,
                                            double h)
 {
-    const double nTa = P.Ta, mC = -P.Cpre;
-    double l, T, k1, k2, k3, k4;
-    l = lam;                      T = fma(beta, lam0 - l, T0); k1 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k1 = is_pos(T) ? k1 : 0.0;
-    l = fma(0.5 * h, k1, lam);    T = fma(beta, lam0 - l, T0); k2 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k2 = is_pos(T) ? k2 : 0.0;
-    l = fma(0.5 * h, k2, lam);    T = fma(beta, lam0 - l, T0); k3 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k3 = is_pos(T) ? k3 : 0.0;
-    l = fma(h, k3, lam);          T = fma(beta, lam0 - l, T0); k4 = l * mC * q_exp_neg(tab, nTa * q_rcp(T)); k4 = is_pos(T) ? k4 : 0.0;
+    double l, k1, k2, k3, k4;
+    l = lam;                      k1 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
+    l = fma(0.5 * h, k1, lam);    k2 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
+    l = fma(0.5 * h, k2, lam);    k3 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
+    l = fma(h, k3, lam);          k4 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
     return fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
 }
 

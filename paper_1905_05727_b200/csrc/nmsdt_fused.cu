@@ -61,12 +61,15 @@ __device__ __forceinline__ double limited_f(double a, double b)
 }
 
 // O4.1-2 for the centre cell W0, given the one-sided differences a = W0 - W(-1), b = W(+1) - W0.
-// R17 first-order fallback (a predicted face density <= 0 -> WL = WR = W0) without a branch: the four densities are
-// predicted first; if one of them is not positive they are replaced by the cell values and the other five slopes are
-// zeroed, which makes their face values equal the cell values exactly (fma(+-0.5, 0, fma(-k, 0, w)) = w).
-template <int LIM>
+// R17 first-order fallback (a predicted face density <= 0 -> WL = WR = W0).  It never fires at CFL 0.4 (nor at 10x that
+// step), so the marching loop does not carry it: EXACT = false only raises `redo` for such a cell, and the caller
+// repeats the warp's whole segment with EXACT = true (the pass is out of place), where the fallback is applied without a
+// branch: the four densities are predicted first; if one of them is not positive they are replaced by the cell values
+// and the other five slopes are zeroed, which makes their face values equal the cell values exactly
+// (fma(+-0.5, 0, fma(-k, 0, w)) = w).
+template <int LIM, bool EXACT>
 __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, const double a[7], const double b[7], double khalf, double WL[7],
-                                           double WR[7])
+                                           double WR[7], bool counted, bool& redo)
 {
     const double w0[7] = {W0.r1, W0.r2, W0.un, W0.ut, W0.p, W0.z1, W0.lam};
     double D[7];
@@ -81,10 +84,14 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
     }
     // all four > 0 (a positive subnormal counts as zero)
     const bool ok = min(min(hi_word(WL[0]), hi_word(WL[1])), min(hi_word(WR[0]), hi_word(WR[1]))) > 0;
-    WL[0] = ok ? WL[0] : w0[0]; WR[0] = ok ? WR[0] : w0[0];
-    WL[1] = ok ? WL[1] : w0[1]; WR[1] = ok ? WR[1] : w0[1];
+    if (EXACT) {
+        WL[0] = ok ? WL[0] : w0[0]; WR[0] = ok ? WR[0] : w0[0];
+        WL[1] = ok ? WL[1] : w0[1]; WR[1] = ok ? WR[1] : w0[1];
 #pragma unroll
-    for (int k = 2; k < 7; ++k) D[k] = ok ? D[k] : 0.0;
+        for (int k = 2; k < 7; ++k) D[k] = ok ? D[k] : 0.0;
+    } else {
+        redo |= counted && !ok;
+    }
     double d[7];
     d[2] = fma(u, D[2], D[4] * W0.irho);
     d[3] = u * D[3];
@@ -99,13 +106,13 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
     }
 }
 
-template <int LIM>
+template <int LIM, bool EXACT>
 __device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, const FCell& W0, const FCell& Wp, double khalf, double WL[7],
-                                           double WR[7])
+                                           double WR[7], bool counted, bool& redo)
 {
     const double a[7] = {W0.r1 - Wm.r1, W0.r2 - Wm.r2, W0.un - Wm.un, W0.ut - Wm.ut, W0.p - Wm.p, W0.z1 - Wm.z1, W0.lam - Wm.lam};
     const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
-    recon_core<LIM>(P, W0, a, b, khalf, WL, WR);
+    recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, counted, redo);
 }
 
 // O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
@@ -225,14 +232,16 @@ constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part
 // free, no barriers): the staged input rows, the primitive window (cells c-2, c-1) and the previous right-face state.
 // Only the half-finished update of cell c-1 stays in registers; this keeps the kernel at 128 registers (16 warps/SM).
 // One column segment of the y-sweep (rows c0 .. c0+seg-1 of column col); returns whether a cell asked for RK4
-// sub-stepping (SRC_FAST only; the caller then redoes the segment with SRC_EXACT -- the pass is out of place).
-template <int MODE, int SRC, int LIM>
+// sub-stepping or the first-order fallback (EXACT = false only; the caller then redoes the segment with EXACT = true --
+// the pass is out of place).
+template <int MODE, bool EXACT, int LIM>
 __device__ __forceinline__ bool y_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
                                           int seg, int col, const double* __restrict__ s_tab, double (*s_q)[7][YT], double (*s_w)[9][YT],
                                           double (*s_r)[YT], double& smax, int& bad)
 {
+    constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
     const int tid = threadIdx.x;
-    bool hot = false;
+    bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
     const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
     const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
@@ -278,7 +287,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
             for (int k = 0; k < 7; ++k) a[k] = s_w[1][k][tid];
             const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
             lam0c = W0.lam;
-            recon_core<LIM>(P, W0, a, b, khalf, WL, WR);
+            recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, jj >= 2, hot);      // rows 0, 1: the window is not real yet
 #pragma unroll
             for (int k = 0; k < 7; ++k) s_w[1][k][tid] = b[k];
         }
@@ -341,13 +350,12 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int col = blockIdx.x * YT + threadIdx.x;
-    constexpr bool HAS_SRC = MODE == MODE_LEAD || MODE == MODE_TRAIL;
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
-        const bool hot = y_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
-        if (HAS_SRC && __any_sync(__activemask(), hot)) {        // rare: redo the warp's segment with the exact R13 rule
+        const bool redo = y_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+        if (__any_sync(__activemask(), redo)) {                  // rare: redo the warp's segment with the exact R13 / R17 rules
             smax = 0.0; bad = 0;
-            y_segment<MODE, SRC_EXACT, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+            y_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
         }
     }
     if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
@@ -357,14 +365,16 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
 // x-sweep (a4): warp per row segment, 2 cells per lane, shared-memory rings between lanes
 // ---------------------------------------------------------------------------------------------------------------
 // One row segment of the x-sweep (cells c0 .. c0+seg-1 of row `row`, one warp); returns whether a cell asked for RK4
-// sub-stepping (SRC_FAST only; the caller then redoes the segment with SRC_EXACT -- the pass is out of place).
-template <int MODE, int SRC, int LIM>
+// sub-stepping or the first-order fallback (EXACT = false only; the caller then redoes the segment with EXACT = true --
+// the pass is out of place).
+template <int MODE, bool EXACT, int LIM>
 __device__ __forceinline__ bool x_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
                                           int seg, int row, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
     double* s_ring = s_dyn;
-    bool hot = false;
+    bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
     double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
     double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
     double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
@@ -429,10 +439,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
             lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
             double WL[7], WR[7];
-            recon_fast<LIM>(P, Wmm, Wm1, WA, khalf, WL, WR);
+            recon_fast<LIM, EXACT>(P, Wmm, Wm1, WA, khalf, WL, WR, k > 0 || lane > 0, hot);   // (k = 0, lane 0: the left slot is not written yet)
             face_fast(P, s_tab, WL, FL1);
             face_fast(P, s_tab, WR, FR1);
-            recon_fast<LIM>(P, Wm1, WA, WB, khalf, WL, WR);
+            recon_fast<LIM, EXACT>(P, Wm1, WA, WB, khalf, WL, WR, k > 0 || lane > 0, hot);
             face_fast(P, s_tab, WL, FL2);
             FFace FR2;
             face_fast(P, s_tab, WR, FR2);
@@ -511,14 +521,13 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int row = blockIdx.x * XW + (threadIdx.x >> 5);
-    constexpr bool HAS_SRC = MODE == MODE_LEAD || MODE == MODE_TRAIL;
     double smax = 0.0; int bad = 0;
     if (row < P.ny) {
-        const bool hot = x_segment<MODE, HAS_SRC ? SRC_FAST : SRC_NONE, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
-        if (HAS_SRC && __any_sync(0xffffffffu, hot)) {           // rare: redo the warp's segment with the exact R13 rule
+        const bool redo = x_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
+        if (__any_sync(0xffffffffu, redo)) {                     // rare: redo the warp's segment with the exact R13 / R17 rules
             smax = 0.0; bad = 0;
             __syncwarp();
-            x_segment<MODE, SRC_EXACT, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
+            x_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
         }
     }
     if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
