@@ -41,7 +41,8 @@ typedef struct sim sim_t;
 
 enum { SIM_OK = 0, SIM_ERR_ARG = -1, SIM_ERR_CUDA = -2, SIM_ERR_STATE = -3, SIM_ERR_BAD = -4 };
 /* boundary kinds (P:129 inflow/transmissive left, P:135 periodic top/bottom; R12) */
-enum { SIM_BC_TRANSMISSIVE = 0, SIM_BC_PERIODIC = 1, SIM_BC_REFLECTIVE = 2, SIM_BC_INFLOW_FIXED = 3 };
+enum { SIM_BC_TRANSMISSIVE = 0, SIM_BC_PERIODIC = 1, SIM_BC_REFLECTIVE = 2, SIM_BC_INFLOW_FIXED = 3,
+       SIM_BC_EXTERNAL = 4 /* x sides only: the two ghost columns belong to a neighbour slab (sim_slab_*) */ };
 /* slope limiter ("van Leer non-smooth slope limiter"; R5): minmod form (default) or monotonised central */
 enum { SIM_LIM_MINMOD = 0, SIM_LIM_MC = 1 };
 /* field ids for sim_read_field */
@@ -149,6 +150,59 @@ int sim_get_cavities(sim_t*, sim_cavity_t* host_out, int cap, int* n);
 int sim_profiles(sim_t*, double p_front, double* host_pbar, double* host_rhobar, double* host_ubar, double* xs_out);
 int sim_qdot_pdf(sim_t*, double n_lo, double dn, int nbins, double* host_mass, long long* host_count);
 int sim_shock_kinematics(sim_t*, const double* host_t, const double* host_xs, int n, double dtau, double* host_us, double* host_as);
+
+/* ---- multi-GPU slab decomposition along x (the paper names multi-GPU runs as future
+ * work).  The domain is cut into slabs of whole columns, one handle (one GPU, one process) per slab.  A side
+ * that faces another slab has the boundary kind SIM_BC_EXTERNAL: the halo step leaves its two ghost columns alone and
+ * the caller fills them with the neighbour's two edge columns before every x-sweep (the only exchange of a step: the
+ * y-sweep and the source step need nothing, stencil radius 2 in x, S8(e)); the time step needs the maximum wavespeed
+ * over all slabs.  A step is driven piecewise (python: paper_1905_05727_b200/slab.py):
+ *
+ *     sim_slab_begin(s, dt_fixed)            local max wavespeed of the state -> the word sim_slab_smax_ptr points to
+ *       <max-allreduce of that 8-byte word over the slabs>   (ordered bits of a non-negative double: integer max)
+ *     sim_slab_ctl(s, 0)                     dt of the first step
+ *     per step, for pass = 1, 2:
+ *         if sim_slab_pass_dir(s, pass) == 0:  exchange: sim_slab_push (peer stores) or pack / transport / unpack
+ *         sim_slab_pass(s, pass)             local halo + fused sweep (pass 2 leaves the new local max wavespeed)
+ *       <max-allreduce>;  sim_slab_ctl(s, 1)   t += dt, step += 1, next dt
+ *
+ * Every slab then computes bit for bit what the single-handle run computes for its columns (same kernels, same dt).
+ * All calls are [async] on the handle's stream unless marked; `pass` is 1 or 2, `side` is 0 (x-lo) or 1 (x-hi).
+ * The exchanged block of one side is 7 planes x ny rows x 2 columns of doubles, dense in that order
+ * (sim_slab_halo_bytes).  Fused variant only. */
+typedef struct {
+    void* plane0[2];            /* DEVICE pointers to plane 0 of the two plane sets (A: state between steps, B: between the passes) */
+    long long plane_stride;     /* doubles between planes */
+    int pitch, nx, ny;          /* doubles per row; interior size of that slab */
+} sim_slab_peer_t;
+
+/* sim_init for the slab whose first interior column is column x_origin of the global domain: `global_init` is the
+   problem setup of the whole domain (shock_cells, cavity list / lattice / generator in global cell units; the seeded
+   generator returns the same list on every slab), painted into this slab's columns. M2tot0 is the slab's share. [sync] */
+int sim_init_slab(sim_t*, const sim_init_t* global_init, int x_origin);
+size_t sim_slab_halo_bytes(const sim_t*);
+int sim_slab_begin(sim_t*, double dt_fixed /* 0 = CFL-limited */);
+int sim_slab_smax_ptr(sim_t*, void** device_word);          /* DEVICE pointer to the unsigned 64-bit max-wavespeed word */
+int sim_slab_ctl(sim_t*, int advance);
+int sim_slab_pass_dir(const sim_t*, int pass);             /* 0 = x, 1 = y for this pass of the current step; <0 on error */
+int sim_slab_pass(sim_t*, int pass);
+/* staging transport (NCCL send/recv, or any other): edge columns of this pass's input state -> dense DEVICE block,
+   dense DEVICE block -> ghost columns of this pass's input state */
+int sim_slab_pack(sim_t*, int pass, int side, void* device_out);
+int sim_slab_unpack(sim_t*, int pass, int side, const void* device_in);
+/* peer-store transport (NVLink / NVSwitch peer memory): describe this slab (sim_slab_info), hand a neighbour's
+   description to sim_slab_connect (its pointers must be valid in this process: same process, or mapped through
+   sim_slab_ipc_*), then sim_slab_push writes this slab's edge columns straight into the connected neighbours' ghost
+   columns.  The caller orders push -> <barrier over the slabs> -> sim_slab_pass. peer = NULL disconnects. */
+int sim_slab_info(const sim_t*, sim_slab_peer_t* out);
+int sim_slab_connect(sim_t*, int side, const sim_slab_peer_t* peer);
+int sim_slab_push(sim_t*, int pass);
+/* CUDA IPC plumbing for the peer-store transport between processes: export the handle of this slab's workspace
+   allocation (64 opaque bytes + the offsets of the two plane sets in it; needs a library-allocated workspace,
+   device_buf = NULL in sim_create), open / close a neighbour's in this process. [sync] */
+int sim_slab_ipc_export(const sim_t*, void* host_handle64, size_t* offset_A, size_t* offset_B);
+int sim_slab_ipc_open(const void* host_handle64, void** device_base);
+int sim_slab_ipc_close(void* device_base);
 
 /* Select kernel variant (SIM_VARIANT_*) and whether sim_step replays CUDA graphs (default on). */
 int sim_set_variant(sim_t*, int variant, int use_graph);

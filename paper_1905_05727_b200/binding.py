@@ -23,7 +23,10 @@ SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
            "sim_read_field", "sim_get_cavities", "sim_set_variant", "sim_launch_count", "sim_device_layout",
            "sim_probe_fp64", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
-           "sim_shock_kinematics"]
+           "sim_shock_kinematics", "sim_init_slab", "sim_slab_halo_bytes", "sim_slab_begin", "sim_slab_smax_ptr",
+           "sim_slab_ctl", "sim_slab_pass_dir", "sim_slab_pass", "sim_slab_pack", "sim_slab_unpack", "sim_slab_info",
+           "sim_slab_connect", "sim_slab_push", "sim_slab_ipc_export", "sim_slab_ipc_open", "sim_slab_ipc_close"]
+BC_EXTERNAL = 4
 KERNEL_KINDS = {"sweep_x": 0, "sweep_y": 1, "source": 2, "cfl": 3, "halo": 4}
 
 
@@ -60,6 +63,11 @@ class Diag(C.Structure):
                 ("M2r", C.c_double), ("M2tot0", C.c_double), ("burned_mass", C.c_double), ("rate_inst", C.c_double),
                 ("mass1", C.c_double), ("mass2", C.c_double), ("momx", C.c_double), ("momy", C.c_double),
                 ("energy", C.c_double), ("bad_state", C.c_int)]
+
+
+class SlabPeer(C.Structure):
+    _fields_ = [("plane0", C.c_void_p * 2), ("plane_stride", C.c_longlong), ("pitch", C.c_int), ("nx", C.c_int),
+                ("ny", C.c_int)]
 
 
 class NmsdtError(RuntimeError):
@@ -108,6 +116,21 @@ def load_library():
         "sim_probe_math": (C.c_int, [vp, C.c_int, dp, C.c_int, C.c_double, C.c_double, dp, dp]),
         "sim_profile": (C.c_int, [vp, C.c_int]),
         "sim_kernel_time": (C.c_int, [vp, C.c_int, dp, C.POINTER(C.c_longlong)]),
+        "sim_init_slab": (C.c_int, [vp, C.POINTER(Init), C.c_int]),
+        "sim_slab_halo_bytes": (C.c_size_t, [vp]),
+        "sim_slab_begin": (C.c_int, [vp, C.c_double]),
+        "sim_slab_smax_ptr": (C.c_int, [vp, C.POINTER(vp)]),
+        "sim_slab_ctl": (C.c_int, [vp, C.c_int]),
+        "sim_slab_pass_dir": (C.c_int, [vp, C.c_int]),
+        "sim_slab_pass": (C.c_int, [vp, C.c_int]),
+        "sim_slab_pack": (C.c_int, [vp, C.c_int, C.c_int, vp]),
+        "sim_slab_unpack": (C.c_int, [vp, C.c_int, C.c_int, vp]),
+        "sim_slab_info": (C.c_int, [vp, C.POINTER(SlabPeer)]),
+        "sim_slab_connect": (C.c_int, [vp, C.c_int, C.POINTER(SlabPeer)]),
+        "sim_slab_push": (C.c_int, [vp, C.c_int]),
+        "sim_slab_ipc_export": (C.c_int, [vp, vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
+        "sim_slab_ipc_open": (C.c_int, [vp, C.POINTER(vp)]),
+        "sim_slab_ipc_close": (C.c_int, [vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -133,7 +156,7 @@ def workspace_bytes(grid):
 class Sim:
     """One simulation on the current CUDA device. grid/eos/kin/init are plain dicts (see `inputs`)."""
 
-    def __init__(self, grid, eos, kin, device=None, variant=None, use_graph=True):
+    def __init__(self, grid, eos, kin, device=None, variant=None, use_graph=True, library_workspace=False):
         import torch
         self.L = load_library()
         if not torch.cuda.is_available():
@@ -149,10 +172,12 @@ class Sim:
             raise NmsdtError("sim_workspace_bytes", SIM_ERR_ARG, "bad grid")
         self.h = C.c_void_p()
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # device memory: torch's
+            # device memory: torch's, unless the workspace must be a cudaMalloc allocation of its own (CUDA IPC export)
+            self.workspace = None if library_workspace else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = torch.cuda.current_stream(self.device)
             rc = self.L.sim_create(C.byref(self.grid), C.byref(self.eos), C.byref(self.kin),
-                                   C.c_void_p(self.workspace.data_ptr()), nbytes, C.c_void_p(self.stream.cuda_stream),
+                                   C.c_void_p(self.workspace.data_ptr() if self.workspace is not None else None),
+                                   nbytes if self.workspace is not None else 0, C.c_void_p(self.stream.cuda_stream),
                                    C.byref(self.h))
         if rc != 0:
             raise NmsdtError("sim_create", rc, (self.L.sim_last_error(None) or b"").decode())
@@ -177,7 +202,8 @@ class Sim:
             pass
 
     # -- the calls of include/nmsdt.h ------------------------------------------------------------------
-    def init(self, init):
+    def init(self, init, x_origin=None):
+        """sim_init, or sim_init_slab when x_origin (global column of this slab's first column) is given"""
         d = dict(init)
         cav = d.pop("cavities", None)
         ini = _fill(Init(), d)
@@ -186,7 +212,10 @@ class Sim:
             keep = (Cavity * len(cav))(*[Cavity(float(c[0]), float(c[1]), float(c[2])) for c in cav])
             ini.cav = C.cast(keep, C.POINTER(Cavity))
             ini.ncav = len(cav)
-        self._chk(self.L.sim_init(self.h, C.byref(ini)), "sim_init")
+        if x_origin is None:
+            self._chk(self.L.sim_init(self.h, C.byref(ini)), "sim_init")
+        else:
+            self._chk(self.L.sim_init_slab(self.h, C.byref(ini), int(x_origin)), "sim_init_slab")
 
     def init_fields(self, q):
         q = [np.ascontiguousarray(a, dtype=np.float64).reshape(self.ny, self.nx) for a in q]
@@ -306,3 +335,51 @@ class Sim:
 
     def synchronize(self):
         self.stream.synchronize()
+
+    # -- slab decomposition (include/nmsdt.h sim_slab_*) ---------------------------------------------------
+    def slab_halo_bytes(self):
+        return int(self.L.sim_slab_halo_bytes(self.h))
+
+    def slab_begin(self, dt_fixed=0.0):
+        self._chk(self.L.sim_slab_begin(self.h, float(dt_fixed)), "sim_slab_begin")
+
+    def slab_smax_ptr(self):
+        p = C.c_void_p()
+        self._chk(self.L.sim_slab_smax_ptr(self.h, C.byref(p)), "sim_slab_smax_ptr")
+        return int(p.value)
+
+    def slab_ctl(self, advance):
+        self._chk(self.L.sim_slab_ctl(self.h, int(bool(advance))), "sim_slab_ctl")
+
+    def slab_pass_dir(self, p):
+        d = self.L.sim_slab_pass_dir(self.h, int(p))
+        if d < 0:
+            raise NmsdtError("sim_slab_pass_dir", d, "bad argument")
+        return d
+
+    def slab_pass(self, p):
+        self._chk(self.L.sim_slab_pass(self.h, int(p)), "sim_slab_pass")
+
+    def slab_pack(self, p, side, dev_ptr):
+        self._chk(self.L.sim_slab_pack(self.h, int(p), int(side), C.c_void_p(dev_ptr)), "sim_slab_pack")
+
+    def slab_unpack(self, p, side, dev_ptr):
+        self._chk(self.L.sim_slab_unpack(self.h, int(p), int(side), C.c_void_p(dev_ptr)), "sim_slab_unpack")
+
+    def slab_info(self):
+        info = SlabPeer()
+        self._chk(self.L.sim_slab_info(self.h, C.byref(info)), "sim_slab_info")
+        return info
+
+    def slab_connect(self, side, peer):
+        self._chk(self.L.sim_slab_connect(self.h, int(side), C.byref(peer) if peer is not None else None), "sim_slab_connect")
+
+    def slab_push(self, p):
+        self._chk(self.L.sim_slab_push(self.h, int(p)), "sim_slab_push")
+
+    def slab_ipc_export(self):
+        """(64-byte handle, offset of plane set A, offset of plane set B) of a library-allocated workspace"""
+        buf = C.create_string_buffer(64)
+        oa, ob = C.c_size_t(), C.c_size_t()
+        self._chk(self.L.sim_slab_ipc_export(self.h, buf, C.byref(oa), C.byref(ob)), "sim_slab_ipc_export")
+        return bytes(buf.raw), int(oa.value), int(ob.value)

@@ -10,7 +10,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnmsdt.so")
-SOURCES = ["nmsdt_step.cu", "nmsdt_fused.cu", "nmsdt_init.cu", "nmsdt_post.cu", "nmsdt_capi.cu"]
+SOURCES = ["nmsdt_step.cu", "nmsdt_fused.cu", "nmsdt_init.cu", "nmsdt_post.cu", "nmsdt_slab.cu", "nmsdt_capi.cu"]
 HEADERS = ["nmsdt_device.cuh", "nmsdt_math.cuh", "nmsdt_fast.cuh", "nmsdt_host.h", os.path.join("..", "..", "include", "nmsdt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v"]

@@ -73,6 +73,8 @@ struct sim {
     double dt_mode = -1.0;          // dt_fixed the control block was last prepared for
     long long launches = 0;
     std::string err;
+    sim_slab_peer_t peer[2];        // slab decomposition: connected neighbours (peer-store transport)
+    bool peer_on[2] = {false, false};
     // event profiling (sim_profile)
     struct EvPair { cudaEvent_t a, b; int kind; };
     std::vector<EvPair> ev;
@@ -101,7 +103,7 @@ bool grid_ok(const sim_grid_t* g)
 {
     if (!g || g->nx < 1 || g->ny < 1 || !(g->dx > 0.0) || !(g->dy > 0.0) || !(g->cfl > 0.0)) return false;
     const int b[4] = {g->bc_xlo, g->bc_xhi, g->bc_ylo, g->bc_yhi};
-    for (int i = 0; i < 4; ++i) if (b[i] < 0 || b[i] > 3) return false;
+    for (int i = 0; i < 4; ++i) if (b[i] < 0 || b[i] > (i < 2 ? SIM_BC_EXTERNAL : 3)) return false;
     if (g->bc_xhi == SIM_BC_INFLOW_FIXED || g->bc_ylo == SIM_BC_INFLOW_FIXED || g->bc_yhi == SIM_BC_INFLOW_FIXED) return false;
     if ((g->bc_xlo == SIM_BC_PERIODIC) != (g->bc_xhi == SIM_BC_PERIODIC)) return false;
     if ((g->bc_ylo == SIM_BC_PERIODIC) != (g->bc_yhi == SIM_BC_PERIODIC)) return false;
@@ -328,28 +330,30 @@ void sim_destroy(sim_t* s)
     delete s;
 }
 
-int sim_init(sim_t* s, const sim_init_t* in)
+// sim_init of the slab whose first interior column is global column x0 (x0 = 0, whole domain: sim_init)
+static int init_common(sim_t* s, const sim_init_t* in, int x0, bool slab)
 {
     if (!s || !in) return fail(s, SIM_ERR_ARG, "sim_init: NULL argument");
-    if (in->shock_cells < 0 || in->shock_cells > s->g.nx || !(in->interface_width > 0.0)) return fail(s, SIM_ERR_ARG, "sim_init: bad shock_cells / interface_width");
+    if (in->shock_cells < 0 || (!slab && in->shock_cells > s->g.nx) || !(in->interface_width > 0.0)) return fail(s, SIM_ERR_ARG, "sim_init: bad shock_cells / interface_width");
     cudaStream_t st = s->stream;
     const Params& P = s->P;
     if (s->d_cav) { cudaFree(s->d_cav); s->d_cav = nullptr; }
     s->ncav = 0;
     std::vector<Cav> host;
     if (in->cav && in->ncav > 0) {
-        for (int i = 0; i < in->ncav; ++i) host.push_back({in->cav[i].x, in->cav[i].y, in->cav[i].r});
+        for (int i = 0; i < in->ncav; ++i) host.push_back({in->cav[i].x - x0, in->cav[i].y, in->cav[i].r});
     } else if (in->lattice) {     // R20: centres x_lo + s/2 + s i, s/2 + s j
         if (!(in->lattice_spacing > 0.0) || !(in->lattice_d > 0.0)) return fail(s, SIM_ERR_ARG, "sim_init: bad lattice");
         const double sp = in->lattice_spacing, r = 0.5 * in->lattice_d;
         for (int jj = 0; sp * (jj + 1) <= (double)s->g.ny; ++jj)
-            for (int ii = 0; in->x_lo + sp * (ii + 1) <= (double)in->x_hi; ++ii) host.push_back({in->x_lo + 0.5 * sp + sp * ii, 0.5 * sp + sp * jj, r});
+            for (int ii = 0; in->x_lo + sp * (ii + 1) <= (double)in->x_hi; ++ii) host.push_back({in->x_lo + 0.5 * sp + sp * ii - x0, 0.5 * sp + sp * jj, r});
     } else if (in->phi > 0.0) {
         int n = generate_cavities(in->seed, in->phi, in->dmin, in->dmax, in->min_gap, in->x_lo, in->x_hi, s->g.ny,
                                   s->g.bc_ylo == SIM_BC_PERIODIC ? 1 : 0, &s->d_cav, st, &s->launches);
         if (n == -1) return fail(s, SIM_ERR_ARG, "sim_init: bad generator parameters");
         if (n < 0) { cudaGetLastError(); return fail(s, SIM_ERR_CUDA, "sim_init: cavity generator failed"); }
         s->ncav = n;
+        if (x0 != 0 && n > 0) { launch_shift_cavities(s->d_cav, n, -(double)x0, st); s->launches++; }
     }
     if (!host.empty()) {
         if (cudaMalloc(&s->d_cav, sizeof(Cav) * host.size()) != cudaSuccess) { cudaGetLastError(); return fail(s, SIM_ERR_CUDA, "sim_init: cudaMalloc"); }
@@ -361,10 +365,14 @@ int sim_init(sim_t* s, const sim_init_t* in)
     if (in->shock_cells > 0 && !hugoniot(s->e, in->p0, in->rho1_0, in->rho2_0, in->p_shock, hug)) return fail(s, SIM_ERR_ARG, "sim_init: Hugoniot solve failed");
     launch_zero_plane(P, s->A + 5 * P.fstride, st);
     launch_paint(P, s->A + 5 * P.fstride, s->d_cav, s->ncav, 0.5 * in->interface_width, st);
-    launch_fill_state(P, s->A, in->shock_cells, hug, in->p_shock, in->p0, in->rho1_0, in->rho2_0, st);
+    const int sc_local = in->shock_cells - x0 < 0 ? 0 : (in->shock_cells - x0 > s->g.nx ? s->g.nx : in->shock_cells - x0);
+    launch_fill_state(P, s->A, sc_local, hug, in->p_shock, in->p0, in->rho1_0, in->rho2_0, st);
     s->launches += 3;
     return finish_init(s);
 }
+
+int sim_init(sim_t* s, const sim_init_t* in) { return init_common(s, in, 0, false); }
+int sim_init_slab(sim_t* s, const sim_init_t* in, int x_origin) { return init_common(s, in, x_origin, true); }
 
 int sim_init_fields(sim_t* s, const double* const host_q[7])
 {
@@ -542,6 +550,159 @@ int sim_device_layout(const sim_t* s, void** plane0, long long* plane_stride, in
     if (pitch) *pitch = s->P.pitch;
     if (x_offset) *x_offset = NGX;
     if (y_offset) *y_offset = NGY;
+    return SIM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// slab decomposition along x (include/nmsdt.h sim_slab_*)
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+// input plane set of a pass of the current step: pass 1 reads A, pass 2 reads B
+double* slab_pass_input(sim* s, int pass) { return pass == 1 ? s->A : s->B; }
+int slab_dir(const sim* s, int pass) { const int d1 = (s->host_step & 1) ? 1 : 0; return pass == 1 ? d1 : 1 - d1; }
+// the two edge columns (ghost = false) or ghost columns (ghost = true) of one x side of a plane set, rows 0..ny-1
+SlabView slab_cols(double* plane0, long long fstride, int pitch, int nx, int side, bool ghost)
+{
+    const int col = side == 0 ? (ghost ? -NG : 0) : (ghost ? nx : nx - NG);
+    return SlabView{plane0 + (long long)NGY * pitch + NGX + col, fstride, (long long)pitch};
+}
+int slab_args(sim* s, int pass, int side, const char* what)
+{
+    if (!s || (pass != 1 && pass != 2) || (side != 0 && side != 1)) return fail(s, SIM_ERR_ARG, std::string(what) + ": bad argument");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, std::string(what) + ": not initialised");
+    if (s->variant != SIM_VARIANT_FUSED) return fail(s, SIM_ERR_STATE, std::string(what) + ": the slab calls drive the fused variant only");
+    if (s->g.nx < NG) return fail(s, SIM_ERR_ARG, std::string(what) + ": a slab needs at least 2 columns");
+    return SIM_OK;
+}
+} // namespace
+
+size_t sim_slab_halo_bytes(const sim_t* s) { return s ? (size_t)7 * s->g.ny * NG * sizeof(double) : 0; }
+
+int sim_slab_begin(sim_t* s, double dt_fixed)
+{
+    if (int rc = slab_args(s, 1, 0, "sim_slab_begin")) return rc;
+    if (dt_fixed < 0.0) return fail(s, SIM_ERR_ARG, "sim_slab_begin: dt_fixed must be >= 0");
+    launch_set_double(&s->ctl->dt_fixed, dt_fixed, s->stream);
+    { KTimer t(s, SIM_K_CFL); launch_cfl(s->P, s->A, s->ctl, s->stream); }
+    s->launches += 2;
+    s->cfl_valid = false;           // sim_step after a slab-driven step recomputes its own dt
+    return check_cuda(s, "sim_slab_begin");
+}
+
+int sim_slab_smax_ptr(sim_t* s, void** device_word)
+{
+    if (!s || !device_word) return fail(s, SIM_ERR_ARG, "sim_slab_smax_ptr: NULL argument");
+    *device_word = &s->ctl->smax_bits;
+    return SIM_OK;
+}
+
+int sim_slab_ctl(sim_t* s, int advance)
+{
+    if (int rc = slab_args(s, 1, 0, "sim_slab_ctl")) return rc;
+    { KTimer t(s, SIM_K_CFL); launch_ctl(s->P, s->ctl, advance ? 1 : 0, s->stream); }
+    s->launches++;
+    if (advance) s->host_step++;
+    return check_cuda(s, "sim_slab_ctl");
+}
+
+int sim_slab_pass_dir(const sim_t* s, int pass)
+{
+    if (!s || (pass != 1 && pass != 2)) return SIM_ERR_ARG;
+    return slab_dir(s, pass);
+}
+
+int sim_slab_pass(sim_t* s, int pass)
+{
+    if (int rc = slab_args(s, pass, 0, "sim_slab_pass")) return rc;
+    const int d = slab_dir(s, pass);
+    double *in = slab_pass_input(s, pass), *out = pass == 1 ? s->B : s->A;
+    { KTimer t(s, SIM_K_HALO); launch_halo(s->P, in, s->inflow, d, s->stream); }
+    { KTimer t(s, d == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(s->P, in, out, &s->ctl->dt, s->ctl, d, pass, s->stream); }
+    s->launches += 2;
+    return check_cuda(s, "sim_slab_pass");
+}
+
+int sim_slab_pack(sim_t* s, int pass, int side, void* device_out)
+{
+    if (int rc = slab_args(s, pass, side, "sim_slab_pack")) return rc;
+    if (!device_out) return fail(s, SIM_ERR_ARG, "sim_slab_pack: NULL buffer");
+    const SlabView src = slab_cols(slab_pass_input(s, pass), s->P.fstride, s->P.pitch, s->g.nx, side, false);
+    const SlabView dst{(double*)device_out, (long long)NG * s->g.ny, (long long)NG};
+    { KTimer t(s, SIM_K_HALO); launch_slab_move(src, dst, s->g.ny, s->stream); }
+    s->launches++;
+    return check_cuda(s, "sim_slab_pack");
+}
+
+int sim_slab_unpack(sim_t* s, int pass, int side, const void* device_in)
+{
+    if (int rc = slab_args(s, pass, side, "sim_slab_unpack")) return rc;
+    if (!device_in) return fail(s, SIM_ERR_ARG, "sim_slab_unpack: NULL buffer");
+    const SlabView src{(double*)device_in, (long long)NG * s->g.ny, (long long)NG};
+    const SlabView dst = slab_cols(slab_pass_input(s, pass), s->P.fstride, s->P.pitch, s->g.nx, side, true);
+    { KTimer t(s, SIM_K_HALO); launch_slab_move(src, dst, s->g.ny, s->stream); }
+    s->launches++;
+    return check_cuda(s, "sim_slab_unpack");
+}
+
+int sim_slab_info(const sim_t* s, sim_slab_peer_t* out)
+{
+    if (!s || !out) return SIM_ERR_ARG;
+    out->plane0[0] = s->A; out->plane0[1] = s->B;
+    out->plane_stride = s->P.fstride; out->pitch = s->P.pitch; out->nx = s->g.nx; out->ny = s->g.ny;
+    return SIM_OK;
+}
+
+int sim_slab_connect(sim_t* s, int side, const sim_slab_peer_t* peer)
+{
+    if (!s || (side != 0 && side != 1)) return fail(s, SIM_ERR_ARG, "sim_slab_connect: bad argument");
+    if (!peer) { s->peer_on[side] = false; return SIM_OK; }
+    if (!peer->plane0[0] || !peer->plane0[1] || peer->ny != s->g.ny || peer->nx < NG || peer->pitch < NGX + peer->nx + NG ||
+        peer->plane_stride < (long long)peer->pitch * (peer->ny + 2 * NGY))
+        return fail(s, SIM_ERR_ARG, "sim_slab_connect: neighbour layout does not fit (same ny, >= 2 columns)");
+    s->peer[side] = *peer; s->peer_on[side] = true;
+    return SIM_OK;
+}
+
+int sim_slab_push(sim_t* s, int pass)
+{
+    if (int rc = slab_args(s, pass, 0, "sim_slab_push")) return rc;
+    const int k = pass == 1 ? 0 : 1;
+    for (int side = 0; side < 2; ++side) {
+        if (!s->peer_on[side]) continue;
+        const sim_slab_peer_t& p = s->peer[side];
+        // my x-lo edge columns are the x-hi ghost columns of my x-lo neighbour, and the other way round
+        const SlabView src = slab_cols(slab_pass_input(s, pass), s->P.fstride, s->P.pitch, s->g.nx, side, false);
+        const SlabView dst = slab_cols((double*)p.plane0[k], p.plane_stride, p.pitch, p.nx, 1 - side, true);
+        { KTimer t(s, SIM_K_HALO); launch_slab_move(src, dst, s->g.ny, s->stream); }
+        s->launches++;
+    }
+    return check_cuda(s, "sim_slab_push");
+}
+
+int sim_slab_ipc_export(const sim_t* s, void* host_handle64, size_t* offset_A, size_t* offset_B)
+{
+    if (!s || !host_handle64 || !offset_A || !offset_B) return SIM_ERR_ARG;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "ipc handle size");
+    if (!s->owns) return fail(const_cast<sim*>(s), SIM_ERR_STATE, "sim_slab_ipc_export: needs a library-allocated workspace (device_buf = NULL)");
+    cudaIpcMemHandle_t h;
+    if (cudaIpcGetMemHandle(&h, s->base) != cudaSuccess) return check_cuda(const_cast<sim*>(s), "sim_slab_ipc_export");
+    std::memcpy(host_handle64, &h, 64);
+    *offset_A = s->L.off_A; *offset_B = s->L.off_B;
+    return SIM_OK;
+}
+
+int sim_slab_ipc_open(const void* host_handle64, void** device_base)
+{
+    if (!host_handle64 || !device_base) return SIM_ERR_ARG;
+    cudaIpcMemHandle_t h; std::memcpy(&h, host_handle64, 64);
+    if (cudaIpcOpenMemHandle(device_base, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) return check_cuda(nullptr, "sim_slab_ipc_open");
+    return SIM_OK;
+}
+
+int sim_slab_ipc_close(void* device_base)
+{
+    if (!device_base) return SIM_ERR_ARG;
+    if (cudaIpcCloseMemHandle(device_base) != cudaSuccess) return check_cuda(nullptr, "sim_slab_ipc_close");
     return SIM_OK;
 }
 

@@ -50,8 +50,13 @@ int launch_qdot_hist(const Params& P, const double* q, double n_lo, double dn, i
                      unsigned long long** d_count, cudaStream_t s);
 int launch_kinematics(const double* d_t, const double* d_xs, int n, double dtau, double* d_us, double* d_as, cudaStream_t s);
 
+// slab decomposition (nmsdt_slab.cu): a block of 7 planes x ny rows x 2 columns inside some strided layout
+struct SlabView { double* base; long long fstride; long long pitch; };
+void launch_slab_move(const SlabView& src, const SlabView& dst, int ny, cudaStream_t s);
+
 // init / output kernels (nmsdt_init.cu)
 void launch_zero_plane(const Params& P, double* plane, cudaStream_t s);
+void launch_shift_cavities(Cav* cav, int n, double shift, cudaStream_t s);
 void launch_paint(const Params& P, double* prof_plane, const Cav* cav, int ncav, double h, cudaStream_t s);
 void launch_fill_state(const Params& P, double* q, int shock_cells, Hug hug, double p_shock, double p0, double rho1_0,
                        double rho2_0, cudaStream_t s);

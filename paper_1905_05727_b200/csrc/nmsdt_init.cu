@@ -49,6 +49,14 @@ void launch_paint(const Params& P, double* prof, const Cav* cav, int ncav, doubl
     if (ncav > 0) k_paint<<<ncav, 256, 0, s>>>(P, prof, cav, ncav, h);
 }
 
+// slab decomposition (sim_init_slab): cavity centres from global to slab-local columns
+__global__ void k_shift_cavities(Cav* __restrict__ cav, int n, double shift)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) cav[k].x += shift;
+}
+void launch_shift_cavities(Cav* cav, int n, double shift, cudaStream_t s) { k_shift_cavities<<<(n + 127) / 128, 128, 0, s>>>(cav, n, shift); }
+
 // ambient state / shocked slab; the painted profile sits in plane 5 on entry
 __global__ void k_fill_state(const __grid_constant__ Params P, double* __restrict__ q, int shock_cells, Hug hug, double p_shock,
                              double p0, double rho1_0, double rho2_0)

@@ -32,8 +32,8 @@ __global__ void k_halo(const __grid_constant__ Params P, double* __restrict__ q,
                 case 2:  w = row[nx - m]; if (f == 2) w = -w; break;
                 default: w = row[nx - 1]; break;
             }
-            row[-m] = v;
-            row[nx - 1 + m] = w;
+            if (P.bc_xlo != 4) row[-m] = v;           // SIM_BC_EXTERNAL: the ghost columns belong to the neighbour slab
+            if (P.bc_xhi != 4) row[nx - 1 + m] = w;
         }
     } else {
         if (t >= P.nx) return;
