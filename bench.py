@@ -9,7 +9,11 @@ resident in HBM; `e2e` = the same metric through the C ABI with HOST buffers (in
 pinned host memory, K steps, diagnostics and all 7 fields read back), copies inside the timed region;
 `roofline` = the dominant kernel (directional sweep) against the FP64-ALU peak (DESIGN.md "Roofline");
 `cpu_baseline` = the oracle timed on this box's host cores on a bounded crop of the same workload.
-The path does not shard (single-GPU method): --gpus N runs N independent replicas ("replicas only").
+BASELINE.json's north_star is a single-GPU method: --gpus N runs N independent replicas ("replicas only")
+by default.  The x-slab decomposition of SURVEY 8(f) NEXT-4 (paper_1905_05727_b200/slab.py) is measured two ways:
+at N = 1 the `slab` block times the same workload cut into 2 slabs on the one GPU (cost of the halo kernels and of the
+piecewise step); `--decomp slab` under torchrun runs ONE domain of N x the workload's columns, one slab per rank, halo
+columns over NCCL send/recv or peer stores (`--transport staged|peer`), dt by a max-allreduce (weak scaling).
 `--impl reference` times the oracle (tests' CPU implementation) instead of the CUDA path.
 """
 import argparse
@@ -147,6 +151,51 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_slab(args, torch, dist, binding, rank, world, local):
+    """one domain of `world` x the workload's columns, one x-slab per rank (weak scaling; DistSlab)"""
+    from paper_1905_05727_b200 import slab
+    K, Wm = max(1, args.steps), max(3, args.warmup)
+    cfg = inputs.config(args.config)
+    g = dict(cfg["grid"])
+    nx1 = g["nx"]
+    g["nx"] = nx1 * world
+    ini = dict(cfg["init"])
+    if ini.get("x_hi"):
+        ini["x_hi"] = g["nx"]
+    mk = lambda sg: binding.Sim(sg, cfg["eos"], cfg["kin"], library_workspace=(args.transport == "peer"))   # noqa: E731
+    ds = slab.DistSlab(g, mk, dist, "cuda:%d" % local, transport=args.transport)
+    ds.init(ini)
+    ds.step(Wm)
+    dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = ds.sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(ds.sim.stream)
+    ds.step(K)
+    e1.record(ds.sim.stream)
+    dist.barrier()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    ms = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+    launches = ds.sim.launch_count() - l0
+    d = ds.diagnostics()
+    cells = g["nx"] * g["ny"]
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": cells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s x %d along x: one domain %dx%d cut into %d x-slabs, halo transport %s, dt by max-allreduce"
+                                   % (args.config, world, g["nx"], g["ny"], world, args.transport),
+                       "parallelism": "x-slabs", "l2_policy": "inputs larger than L2"},
+            "clocks": sampler.summary(), "e2e": None, "gpu_launches": int(launches),
+            "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "M2r": d["M2r"]}}))
+    ds.close()
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -157,6 +206,9 @@ def main():
     ap.add_argument("--variant", type=int, default=1)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-slab", action="store_true")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"])
+    ap.add_argument("--transport", default="staged", choices=["staged", "peer"])
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -174,6 +226,8 @@ def main():
     if world > 1:
         dist.init_process_group("nccl")
     K, Wm = max(1, args.steps), max(3, args.warmup)
+    if args.decomp == "slab" and world > 1:
+        return run_slab(args, torch, dist, binding, rank, world, local)
 
     cfg = inputs.config(args.config, seed=inputs.config(args.config)["init"]["seed"] + rank if args.config in ("C4", "C5") else None)
     g = cfg["grid"]
@@ -279,6 +333,25 @@ def main():
                "job": "sim_init_fields(host) + sim_step(%d) + sim_diagnostics + 7 x sim_read_field(host)" % K, "seconds": el,
                "M2r": de["M2r"]}
 
+    # ---- the same workload cut into 2 x-slabs on this one GPU: cost of the decomposed step ------------
+    slab_block = None
+    if not args.no_slab and world == 1:
+        from paper_1905_05727_b200 import slab
+        sim.close()
+        torch.cuda.empty_cache()
+        ls = slab.LocalSlabs(g, cfg["eos"], cfg["kin"], 2, transport="peer")
+        ls.init(cfg["init"])
+        ls.step(Wm)
+        torch.cuda.synchronize()
+        e0.record(ls.sims[0].stream)
+        ls.step(K)
+        e1.record(ls.sims[0].stream)
+        torch.cuda.synchronize()
+        sms = e0.elapsed_time(e1) / K
+        slab_block = {"slabs": 2, "transport": "peer stores (same device)", "ms_per_step": sms, "vs_undivided": sms / (ms / K),
+                      "halo_bytes_per_step": 2 * ls.sims[0].slab_halo_bytes()}
+        ls.close()
+
     if rank != 0:
         return
     cpu = None
@@ -294,7 +367,7 @@ def main():
                    "variant": args.variant, "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "burned_mass": d["burned_mass"]},
-        "post": post,
+        "post": post, "slab": slab_block,
     }
     print(json.dumps(out))
     if world > 1:

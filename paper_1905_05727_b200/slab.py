@@ -75,23 +75,32 @@ def _as_tensor(ptr, nbytes, dtype, torch, device):
     return torch.from_numpy(arr).view(dtype)
 
 
-def exchange_staged(sim, p, lo, hi, send, recv, dist, group=None):
+def exchange_staged(sim, p, lo, hi, send, recv, dist, group=None, bounce=None):
     """One halo exchange for pass `p`: pack both edges, post all sends / receives at once, unpack the ghosts.
     send / recv: {side: tensor}.  Receives are posted hi first: with two ranks and periodic x both neighbours are the
-    same rank, whose first send (its lo edge) is this rank's hi ghost block (NCCL matches point-to-point in order)."""
+    same rank, whose first send (its lo edge) is this rank's hi ghost block (NCCL matches point-to-point in order).
+    bounce: {("s"|"r", side): CPU tensor} when the backend cannot move device tensors (gloo point-to-point): the blocks
+    then travel through host memory."""
     ops = []
     for side, peer in ((0, lo), (1, hi)):
         if peer is not None:
             sim.slab_pack(p, side, send[side].data_ptr())
-            ops.append(dist.P2POp(dist.isend, send[side], peer, group=group, tag=side))
+            buf = send[side]
+            if bounce is not None:
+                bounce[("s", side)].copy_(send[side])                    # synchronises with the pack kernel
+                buf = bounce[("s", side)]
+            ops.append(dist.P2POp(dist.isend, buf, peer, group=group, tag=side))
     for side, peer in ((1, hi), (0, lo)):
         if peer is not None:
-            ops.append(dist.P2POp(dist.irecv, recv[side], peer, group=group, tag=1 - side))
+            buf = recv[side] if bounce is None else bounce[("r", side)]
+            ops.append(dist.P2POp(dist.irecv, buf, peer, group=group, tag=1 - side))
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
     for side, peer in ((0, lo), (1, hi)):
         if peer is not None:
+            if bounce is not None:
+                recv[side].copy_(bounce[("r", side)])
             sim.slab_unpack(p, side, recv[side].data_ptr())
 
 
@@ -118,6 +127,9 @@ class DistSlab:
         self.smax = _as_tensor(self.sim.slab_smax_ptr(), 8, torch.int64, torch, self.device)
         self.token = torch.zeros(1, dtype=torch.int64, device=self.device)                 # barrier word of the peer transport
         self.transport = transport
+        self.bounce = None
+        if self.device.type == "cuda" and dist.get_backend(group) == "gloo":     # gloo point-to-point moves host memory only
+            self.bounce = {(k, s): torch.empty(nb // 8, dtype=torch.float64).pin_memory() for k in "sr" for s in self.send}
         self._ipc_open = []
         if transport == "peer" and self.world > 1:
             self._connect_peers()
@@ -165,7 +177,7 @@ class DistSlab:
         if self.world == 1:
             return
         if self.transport == "staged":
-            exchange_staged(self.sim, p, self.lo, self.hi, self.send, self.recv, self.dist, self.group)
+            exchange_staged(self.sim, p, self.lo, self.hi, self.send, self.recv, self.dist, self.group, self.bounce)
         else:
             # every rank stores its edge columns into its neighbours' ghost columns, then all ranks meet: when the
             # allreduce has finished on this stream, the neighbours' push kernels (enqueued before theirs) are complete.

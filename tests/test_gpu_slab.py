@@ -112,6 +112,7 @@ def test_decomposed_step_against_the_oracle(O, B):
     for s, (x0, n) in zip(many.sims, many.parts):
         s.init_fields([a[:, x0:x0 + n] for a in q0])
     many._begun = None
+    t0 = o.diagnostics()["t"]                    # init_fields restarts the slabs' clock at 0
     dt = o.cfl_dt()
     o.step_dt(1, dt), many.step(1, dt_fixed=dt)
     r = rel_diff(many.state(), o.state(), o.read_field("c"))
@@ -119,7 +120,7 @@ def test_decomposed_step_against_the_oracle(O, B):
     o.step(20), many.step(20)
     r = l1_rel(many.state(), o.state())
     assert max(r) <= 1e-9, r
-    assert many.diagnostics()["t"] == pytest.approx(o.diagnostics()["t"], rel=1e-12)
+    assert many.diagnostics()["t"] == pytest.approx(o.diagnostics()["t"] - t0, rel=1e-10)
 
 
 def test_slab_argument_checks(B):
