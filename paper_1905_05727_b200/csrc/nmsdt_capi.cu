@@ -38,7 +38,7 @@ Layout make_layout(int nx, int ny)
     L.off_diag = o; o = align_up(o + sizeof(DiagOut), 256);
     L.off_ctl = o; o = align_up(o + sizeof(Ctl), 256);
     L.off_scratch = o; o = align_up(o + 8 * sizeof(double), 256);
-    L.off_tab = o; o = align_up(o + MATH_TAB_DOUBLES * sizeof(double), 256);
+    L.off_tab = o; o = align_up(o + MATH_TAB_DOUBLES_LOG * sizeof(double), 256);
     L.total = o;
     return L;
 }
@@ -124,6 +124,7 @@ void fill_params(sim* s)
     P.kA = -e.A / (1.0 - e.C); P.kB = e.B / (1.0 - e.D); P.AC = e.A * e.C; P.BD = e.B * e.D;
     P.z_min = e.z_min; P.z_max = 1.0 - e.z_min;
     P.C2 = e.C * LOG2E; P.D2 = e.D * LOG2E; P.iG2cv2 = 1.0 / (e.Gamma2 * e.cv2); P.tab = s->tab;
+    fill_pow_coef(P.pw, e.C, e.D);
     P.Ta = k.Ta; P.Cpre = k.Cpre; P.Q = k.Q; P.theta0 = k.substep_theta; P.reactive = k.reactive; P.max_substeps = k.max_substeps;
 }
 
@@ -308,8 +309,8 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     init_fused_kernels();
     cudaMemsetAsync(s->base, 0, s->L.total, s->stream);
     {
-        double htab[MATH_TAB_DOUBLES];
-        fill_math_tables(htab);
+        double htab[MATH_TAB_DOUBLES_LOG];
+        fill_math_tables(htab, e->C, e->D);
         cudaMemcpyAsync(s->tab, htab, sizeof(htab), cudaMemcpyHostToDevice, s->stream);   // pageable source: staged before return
     }
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) { int rc = check_cuda(nullptr, "sim_create"); sim_destroy(s); return rc ? rc : SIM_ERR_CUDA; }
@@ -805,8 +806,8 @@ int sim_shock_kinematics(sim_t* s, const double* host_t, const double* host_xs, 
 
 int sim_probe_math(sim_t* s, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1)
 {
-    if (!s || !host_x || !host_y0 || !host_y1 || n < 1 || fn < 0 || fn > 6) return fail(s, SIM_ERR_ARG, "sim_probe_math: bad argument");
-    if (launch_probe_math(s->P.tab, fn, host_x, n, a, b, host_y0, host_y1, s->stream)) return fail(s, SIM_ERR_CUDA, "sim_probe_math failed");
+    if (!s || !host_x || !host_y0 || !host_y1 || n < 1 || fn < 0 || fn > 7) return fail(s, SIM_ERR_ARG, "sim_probe_math: bad argument");
+    if (launch_probe_math(s->P.pw, s->P.tab, fn, host_x, n, a, b, host_y0, host_y1, s->stream)) return fail(s, SIM_ERR_CUDA, "sim_probe_math failed");
     s->launches += 1;
     return SIM_OK;
 }

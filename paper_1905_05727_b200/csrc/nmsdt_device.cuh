@@ -5,6 +5,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include "nmsdt_math.cuh"
 
 namespace nmsdt {
 
@@ -27,6 +28,7 @@ struct Params {
     int reactive, max_substeps;
     // fused path (nmsdt_fused.cu): C log2(e), D log2(e), 1/(Gamma2 cv2), device copy of the nmsdt_math.cuh tables
     double C2, D2, iG2cv2;
+    PowCoef pw;                  // exponents C, D of Eq. 3-4 and their binomial coefficients (q_pow_tab)
     const double* tab;
 };
 

@@ -31,36 +31,39 @@ __device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
     return (r >= (double)(P.max_substeps - 1)) ? P.max_substeps : 1 + (int)r;
 }
 
-// Arrhenius rate of Eq. 6 at (l, T): -l C exp(-Ta/T) for T > 0, else 0 (O5).  One range test on the high word of
-// y = Ta/T covers both guards: y in [0, 690) <=> T > 0 and exp(-y) above ~1e-300 (the rate is taken as 0 beyond
-// that; 690 = 0x40859000_00000000); T <= 0, T = +0 (y = inf) and NaN all fail the unsigned compare.
-__device__ __forceinline__ double arr_rate(const Params& P, const double* __restrict__ tab, double l, double T)
+// Arrhenius factor of Eq. 6 at (l, T): l exp(-Ta/T) for T > 0, else 0 (O5); the rate is -C times this.  One range test
+// on the high word of y = Ta/T covers both guards: y in [0, 690) <=> T > 0 and exp(-y) above ~1e-300 (the rate is taken
+// as 0 beyond that; 690 = 0x40859000_00000000); T <= 0, T = +0 (y = inf) and NaN all fail the unsigned compare.
+__device__ __forceinline__ double arr_factor(const Params& P, const double* __restrict__ tab, double l, double T)
 {
     const double y = P.Ta * q_rcp(T);
     const bool good = (unsigned)hi_word(y) < 0x40859000u;
-    const double k = l * -P.Cpre * q_exp2_prod(tab, y, -KC[9]);
+    const double k = l * q_exp2_prod(tab, y, -KC[9]);
     return good ? k : 0.0;
 }
 
-// one classic RK4 step of d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)), T2 = T0 + beta (lam0 - lambda), from lam over h
-__device__ __forceinline__ double rk4_step(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double lam,
-                                           double h)
+// one classic RK4 step of d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)), T2 = T0 + beta (lam0 - lambda), from lam over h.
+// The constant -C rides on the step (hC = -h C, stages k_i / (-C)) and T2 = Tb - beta lambda with Tb = T0 + beta lam0:
+// 8 FP64 instructions fewer than the literal form, same values up to rounding.
+__device__ __forceinline__ double rk4_step(const Params& P, const double* __restrict__ tab, double Tb, double beta, double lam, double h)
 {
+    const double hC = -h * P.Cpre, nb = -beta;
     double l, k1, k2, k3, k4;
-    l = lam;                      k1 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
-    l = fma(0.5 * h, k1, lam);    k2 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
-    l = fma(0.5 * h, k2, lam);    k3 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
-    l = fma(h, k3, lam);          k4 = arr_rate(P, tab, l, fma(beta, lam0 - l, T0));
-    return fma(h * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
+    l = lam;                       k1 = arr_factor(P, tab, l, fma(nb, l, Tb));
+    l = fma(0.5 * hC, k1, lam);    k2 = arr_factor(P, tab, l, fma(nb, l, Tb));
+    l = fma(0.5 * hC, k2, lam);    k3 = arr_factor(P, tab, l, fma(nb, l, Tb));
+    l = fma(hC, k3, lam);          k4 = arr_factor(P, tab, l, fma(nb, l, Tb));
+    return fma(hC * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
 }
 
 // R13 sub-stepped integration (only reached by cells hotter than the safe bound)
 __device__ __noinline__ double rk4_substepped(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0, double tau)
 {
-    const int nsub = nsub_exact(P, fma(beta, lam0, T0), tau);
+    const double Tb = fma(beta, lam0, T0);
+    const int nsub = nsub_exact(P, Tb, tau);
     const double h = tau / (double)nsub;
     double lam = lam0;
-    for (int s = 0; s < nsub; ++s) lam = rk4_step(P, tab, T0, beta, lam0, lam, h);
+    for (int s = 0; s < nsub; ++s) lam = rk4_step(P, tab, Tb, beta, lam, h);
     return lam;
 }
 
@@ -75,8 +78,9 @@ template <int SRC>
 __device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* __restrict__ tab, double T0, double beta, double lam0,
                                                 double tau, double Tsafe, bool& hot)
 {
-    double lam = rk4_step(P, tab, T0, beta, lam0, lam0, tau);
-    const bool h = fma(beta, lam0, T0) >= Tsafe;
+    const double Tb = fma(beta, lam0, T0);
+    double lam = rk4_step(P, tab, Tb, beta, lam0, tau);
+    const bool h = Tb >= Tsafe;
     if (SRC == SRC_FAST) {
         hot |= h;
     } else {
@@ -88,11 +92,25 @@ __device__ __forceinline__ double arrhenius_rk4(const Params& P, const double* _
     return dmin_(nonneg(lam), lam0);
 }
 
+// (x^C, x^D) of Eq. 3-4 for x = rho2/rho02 by the table route.  x outside the binade table (never on a physical state):
+// EX = false only raises `oor` (the sweeps then redo the segment with EX = true), EX = true takes the library powers
+// behind a branch.
+template <bool EX>
+__device__ __forceinline__ void eos_pow(const Params& P, const double* __restrict__ tab, double x, double& xC, double& xD, bool& oor)
+{
+    const bool in = q_pow_tab(tab, P.pw, x, xC, xD);
+    if (EX) {
+        if (!in) { xC = pow(x, P.C); xD = pow(x, P.D); }
+    } else {
+        oor |= !in;
+    }
+}
+
 // O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.
 // SRC: the Arrhenius step over tau is applied to the cell; dE = energy moved into rho E, q6n = new z2 rho2 lambda.
 // The kernels that apply the source are only launched for reactive runs (launch_sweep_fused), so there is no
 // P.reactive test here.
-template <int SRC>
+template <int SRC, bool EX = true>
 __device__ __forceinline__ void prim_cell(const Params& P, const double* __restrict__ tab, const double q[7], double tau, double Tsafe,
                                           FCell& W, double& dE, double& q6n, bool& hot)
 {
@@ -110,7 +128,7 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     const double rhoe = fma(-0.5 * irho, fma(q[2], q[2], q[3] * q[3]), q[4]);
     const double x = W.r2 * P.irho02;
     double xC, xD;
-    q_pow_pair(tab, x, P.C2, P.D2, xC, xD);
+    eos_pow<EX>(P, tab, x, xC, xD, hot);
     const double pr = fma(P.A, xC, -P.B * xD);                                   // Eq. 3
     const double rer = fma(P.kA, xC - x, P.kB * (xD - x));                       // rho2 * Eq. 4
     const double xi = fma(z1, P.iG1, z2 * P.iG2);

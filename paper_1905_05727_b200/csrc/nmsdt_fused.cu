@@ -28,7 +28,8 @@ enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2, MODE_TRAIL_INERT = 3 };
 
 struct FFace { double r1, r2, un, ut, p, z1, lam, rho, rhoE, c; };
 
-__device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f)
+template <bool EX>
+__device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f, bool& oor)
 {
     const double z1 = W[5], z2 = 1.0 - z1, p = W[4];
     f.r1 = W[0]; f.r2 = W[1]; f.un = W[2]; f.ut = W[3]; f.p = p; f.z1 = z1; f.lam = W[6];
@@ -36,7 +37,7 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     f.rho = rho;
     const double x = W[1] * P.irho02;
     double xC, xD;
-    q_pow_pair(tab, x, P.C2, P.D2, xC, xD);
+    eos_pow<EX>(P, tab, x, xC, xD, oor);
     const double pr = fma(P.A, xC, -P.B * xD);
     const double rer = fma(P.kA, xC - x, P.kB * (xD - x));
     const double kin = 0.5 * rho * fma(W[2], W[2], W[3] * W[3]);
@@ -160,12 +161,12 @@ __device__ __forceinline__ bool all_finite7(const double o[7])
 }
 
 // finished cell of the second pass: trailing S(dt/2) (SRC != SRC_NONE), wavespeed of the new state, state check (a6, a7, R17)
-template <int SRC>
+template <int SRC, bool EX>
 __device__ __forceinline__ void trail_cell(const Params& P, const double* __restrict__ tab, double o[7], double tau, double Tsafe, double& smax,
                                            int& bad, bool& hot)
 {
     FCell W; double dE, q6n;
-    prim_cell<SRC>(P, tab, o, tau, Tsafe, W, dE, q6n, hot);
+    prim_cell<SRC, EX>(P, tab, o, tau, Tsafe, W, dE, q6n, hot);
     o[4] += dE; o[6] = q6n;
     const double a = dmax_(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
     const bool ok = all_finite7(o) && o[0] > 0.0 && o[1] > 0.0 && (__double2hiint(a) & 0x7fffffff) < 0x7ff00000;
@@ -273,7 +274,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
 #pragma unroll
             for (int k = 0; k < 7; ++k) q[k] = s_q[st][k][tid];
             double dE, q6n;
-            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n, hot);
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n, hot);
         }
         // The body is branch free: during the 4 ramp-up rows it runs on not-yet-valid window / face / flux values
         // (finite or not, never stored: the store and the wavespeed contribution are predicated on jj >= 4).
@@ -294,8 +295,10 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
         s_w[0][0][tid] = Wp.r1; s_w[0][1][tid] = Wp.r2; s_w[0][2][tid] = Wp.un; s_w[0][3][tid] = Wp.ut; s_w[0][4][tid] = Wp.p;
         s_w[0][5][tid] = Wp.z1; s_w[0][6][tid] = Wp.lam; s_w[0][7][tid] = Wp.irho; s_w[0][8][tid] = Wp.rc2;
         FFace fl, fr, pr;
-        face_fast(P, s_tab, WL, fl);
-        face_fast(P, s_tab, WR, fr);
+        bool oor = false;                         // a face density outside the power tables (only counted once the window is real)
+        face_fast<EXACT>(P, s_tab, WL, fl, oor);
+        face_fast<EXACT>(P, s_tab, WR, fr, oor);
+        hot |= oor && jj >= 2;
         pr.r1 = s_r[0][tid]; pr.r2 = s_r[1][tid]; pr.un = s_r[2][tid]; pr.ut = s_r[3][tid]; pr.p = s_r[4][tid];
         pr.z1 = s_r[5][tid]; pr.lam = s_r[6][tid]; pr.rho = s_r[7][tid]; pr.rhoE = s_r[8][tid]; pr.c = s_r[9][tid];
         s_r[0][tid] = fr.r1; s_r[1][tid] = fr.r2; s_r[2][tid] = fr.un; s_r[3][tid] = fr.ut; s_r[4][tid] = fr.p;
@@ -311,7 +314,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
             const bool valid = jj >= 4;
             if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
                 double sm1 = 0.0; int bad1 = 0; bool hot1 = false;
-                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE>(P, s_tab, o, tau, Tsafe, sm1, bad1, hot1);
+                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE, EXACT>(P, s_tab, o, tau, Tsafe, sm1, bad1, hot1);
                 smax = valid ? dmax_(smax, sm1) : smax;
                 bad |= valid ? bad1 : 0;
                 hot |= valid && hot1;
@@ -418,8 +421,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
 #pragma unroll
             for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
             double dE, q6n;
-            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
-            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n, hot);
+            bool hotb = false;                       // cell Ac + 1 = nx + 2 (odd nx) is row padding, not a cell
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n, hotb);
+            hot |= hotb && Ac <= P.nx;
             rw[0 * RING + sw] = WA.r1; rw[1 * RING + sw] = WA.r2; rw[2 * RING + sw] = WA.un; rw[3 * RING + sw] = WA.ut;
             rw[4 * RING + sw] = WA.p;  rw[5 * RING + sw] = WA.z1; rw[6 * RING + sw] = WA.lam;
             rw[7 * RING + sw] = WB.r1; rw[8 * RING + sw] = WB.r2; rw[9 * RING + sw] = WB.un; rw[10 * RING + sw] = WB.ut;
@@ -439,13 +444,15 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
             lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
             double WL[7], WR[7];
+            bool oor = false;                        // a face density outside the power tables
             recon_fast<LIM, EXACT>(P, Wmm, Wm1, WA, khalf, WL, WR, k > 0 || lane > 0, hot);   // (k = 0, lane 0: the left slot is not written yet)
-            face_fast(P, s_tab, WL, FL1);
-            face_fast(P, s_tab, WR, FR1);
+            face_fast<EXACT>(P, s_tab, WL, FL1, oor);
+            face_fast<EXACT>(P, s_tab, WR, FR1, oor);
             recon_fast<LIM, EXACT>(P, Wm1, WA, WB, khalf, WL, WR, k > 0 || lane > 0, hot);
-            face_fast(P, s_tab, WL, FL2);
+            face_fast<EXACT>(P, s_tab, WL, FL2, oor);
             FFace FR2;
-            face_fast(P, s_tab, WR, FR2);
+            face_fast<EXACT>(P, s_tab, WR, FR2, oor);
+            hot |= oor && (k > 0 || lane > 0);
             rfr[0 * RING + sw] = FR2.r1; rfr[1 * RING + sw] = FR2.r2; rfr[2 * RING + sw] = FR2.un; rfr[3 * RING + sw] = FR2.ut;
             rfr[4 * RING + sw] = FR2.p;  rfr[5 * RING + sw] = FR2.z1; rfr[6 * RING + sw] = FR2.lam; rfr[7 * RING + sw] = FR2.rho;
             rfr[8 * RING + sw] = FR2.rhoE; rfr[9 * RING + sw] = FR2.c;
@@ -487,8 +494,8 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             const bool two = u0 + 1 < c1;
             if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
                 double sm1 = 0.0, sm2 = 0.0; int bad1 = 0, bad2 = 0; bool hot1 = false, hot2 = false;
-                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE>(P, s_tab, oa, tau, Tsafe, sm1, bad1, hot1);
-                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE>(P, s_tab, ob, tau, Tsafe, sm2, bad2, hot2);
+                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE, EXACT>(P, s_tab, oa, tau, Tsafe, sm1, bad1, hot1);
+                trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE, EXACT>(P, s_tab, ob, tau, Tsafe, sm2, bad2, hot2);
                 sm1 = valid ? sm1 : 0.0; sm2 = (valid && two) ? sm2 : 0.0;
                 smax = dmax_(smax, dmax_(sm1, sm2));
                 bad |= (valid ? bad1 : 0) | ((valid && two) ? bad2 : 0);
@@ -689,11 +696,11 @@ double host_tsafe(double tau, double Cpre, double Ta, double theta0) { return ts
 // ---------------------------------------------------------------------------------------------------------------
 // sim_probe_math: evaluate the elementary functions of nmsdt_math.cuh on device arrays (accuracy tests)
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_probe_math(const double* __restrict__ tab_g, int fn, const double* __restrict__ x, int n, double a, double b,
+__global__ void __launch_bounds__(128) k_probe_math(const __grid_constant__ PowCoef pw, const double* __restrict__ tab_g, int fn, const double* __restrict__ x, int n, double a, double b,
                                                     double* __restrict__ y0, double* __restrict__ y1)
 {
-    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
-    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = tab_g[i];
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES_LOG];
+    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES_LOG; i += blockDim.x) s_tab[i] = tab_g[i];
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -707,19 +714,20 @@ __global__ void __launch_bounds__(128) k_probe_math(const double* __restrict__ t
     case 4: r0 = q_exp_neg(s_tab, v); break;
     case 5: r0 = floor1(v); r1 = clamp01(v); break;
     case 6: r0 = nonneg(v); r1 = cap690(v); break;
+    case 7: if (!q_pow_tab(s_tab, pw, v, r0, r1)) { r0 = pow(v, pw.C); r1 = pow(v, pw.D); } break;   // the step kernels' route for Eq. 3-4
     default: break;
     }
     y0[i] = r0; y1[i] = r1;
 }
 
-int launch_probe_math(const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
+int launch_probe_math(const PowCoef& pw, const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
                       cudaStream_t s)
 {
     double *dx = nullptr, *dy = nullptr;
     if (cudaMalloc(&dx, sizeof(double) * n) != cudaSuccess) return -2;
     if (cudaMalloc(&dy, sizeof(double) * 2 * n) != cudaSuccess) { cudaFree(dx); return -2; }
     cudaMemcpyAsync(dx, host_x, sizeof(double) * n, cudaMemcpyHostToDevice, s);
-    k_probe_math<<<(n + 127) / 128, 128, 0, s>>>(tab_dev, fn, dx, n, a, b, dy, dy + n);
+    k_probe_math<<<(n + 127) / 128, 128, 0, s>>>(pw, tab_dev, fn, dx, n, a, b, dy, dy + n);
     cudaMemcpyAsync(host_y0, dy, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
     cudaMemcpyAsync(host_y1, dy + n, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
     const cudaError_t e = cudaStreamSynchronize(s);

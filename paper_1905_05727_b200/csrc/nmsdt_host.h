@@ -36,7 +36,7 @@ void launch_sweep_fused(const Params& P, const double* qin, double* qout, const 
 void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s);
 void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s);
 double host_tsafe(double tau, double Cpre, double Ta, double theta0);
-int  launch_probe_math(const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
+int  launch_probe_math(const PowCoef& pw, const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
                        cudaStream_t s);
 
 // post-processing (nmsdt_post.cu): Eq. 9-11 profiles + front position, Eq. 14-16 histogram, Eq. C1-C2 kinematics.

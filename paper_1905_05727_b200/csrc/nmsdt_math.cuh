@@ -23,9 +23,14 @@
 
 namespace nmsdt {
 
-constexpr int LOG_TAB_BITS = 8, LOG_TAB_N = 1 << LOG_TAB_BITS;     // (1/c_j, ln c_j) pairs
+constexpr int LOG_TAB_BITS = 8, LOG_TAB_N = 1 << LOG_TAB_BITS;     // c_j = 1 + (j + 1/2)/256: 1/c_j, ln c_j, c_j^C, c_j^D
 constexpr int EXP_TAB_BITS = 8, EXP_TAB_N = 1 << EXP_TAB_BITS;     // 2^(j/256)
-constexpr int MATH_TAB_DOUBLES = 2 * LOG_TAB_N + EXP_TAB_N;        // 768 doubles = 6144 B of shared memory
+constexpr int POW_E_MIN = -8, POW_E_N = 16;                        // binades 2^-8 .. 2^7 of the table-driven powers
+// table layout (doubles): [1/c_j][2^(j/256)][(c_j^C, c_j^D)][(2^(eC), 2^(eD))] | [ln c_j]
+constexpr int IC_OFF = 0, EXP_OFF = LOG_TAB_N, POW_OFF = EXP_OFF + EXP_TAB_N, PE_OFF = POW_OFF + 2 * LOG_TAB_N;
+constexpr int LC_OFF = PE_OFF + 2 * POW_E_N;
+constexpr int MATH_TAB_DOUBLES = LC_OFF;                           // 1056 doubles = 8448 B: what the step kernels hold in shared memory
+constexpr int MATH_TAB_DOUBLES_LOG = LC_OFF + LOG_TAB_N;           // + ln c_j for the kernels that call q_log (post-processing, probe)
 
 #if defined(__CUDA_ARCH__)
 #define NMSDT_HD __device__ __forceinline__
@@ -92,14 +97,15 @@ NMSDT_HD double nonneg(double x) { return hi_word(x) < 0 ? 0.0 : x; }
 NMSDT_HD double clamp01(double x) { const int h = hi_word(x); return h < 0 ? 0.0 : (h >= 0x3ff00000 ? 1.0 : x); }
 NMSDT_HD double cap690(double y) { return hi_word(y) < 0x40859000 ? y : 690.0; }
 
-// ln(x), x positive normal.  tab = shared-memory copy of the tables.  Absolute error ~1e-16 (+ 1 ulp of the result).
+// ln(x), x positive normal.  tab = shared-memory copy of the tables INCLUDING the ln c_j part (MATH_TAB_DOUBLES_LOG).
+// Absolute error ~1e-16 (+ 1 ulp of the result).
 NMSDT_HD double q_log(const double* __restrict__ tab, double x)
 {
     const int hx = hi_word(x);
     const int j = (hx >> (20 - LOG_TAB_BITS)) & (LOG_TAB_N - 1);
     const double m = mk_double((hx & 0x000fffff) | 0x3ff00000, lo_word(x));            // mantissa in [1,2)
     const double ed = mk_double(0x43300000, hx >> 20) - 4503599627371519.0;             // unbiased exponent: (2^52 + e_biased) - (2^52 + 1023)
-    const double ic = tab[2 * j], lc = tab[2 * j + 1];
+    const double ic = tab[IC_OFF + j], lc = tab[LC_OFF + j];
     const double r = fma(m, ic, -1.0);                                                 // |r| <= 2^-9: r^6/6 < 1e-17
     double p = fma(r, KC[1], -0.25);
     p = fma(p, r, KC[2]);
@@ -115,7 +121,7 @@ NMSDT_HD double q_exp2_prod(const double* __restrict__ tab, double a, double b)
     const double t = fma(a, b, SH);
     const int N = lo_word(t);
     const double f = fma(a, b, -(t - SH));                      // |f| <= 1/512: (f ln2)^5/120 < 4e-17
-    const double T = tab[2 * LOG_TAB_N + (N & (EXP_TAB_N - 1))];
+    const double T = tab[EXP_OFF + (N & (EXP_TAB_N - 1))];
     double p = fma(f, KC[5], KC[6]);
     p = fma(p, f, KC[7]);
     p = fma(p, f, KC[8]);
@@ -125,7 +131,34 @@ NMSDT_HD double q_exp2_prod(const double* __restrict__ tab, double a, double b)
 
 constexpr double LOG2E = 1.4426950408889634074;
 
-// (x^C, x^D) from one logarithm; C2 = C*log2(e), D2 = D*log2(e)
+// (x^C, x^D) for the two fixed exponents of Eq. 3-4 without a logarithm: x = 2^e c_j (1 + r), |r| <= 2^-9, so
+//   x^C = 2^(eC) c_j^C (1 + r)^C,  (1 + r)^C = 1 + r (C + r (b2 + r (b3 + r (b4 + r b5)))),  b_k = binom(C, k)
+// (next term binom(C,6) r^6 < 2e-18).  Two table products + 5 DFMA per power, 15 FP64 instructions for the pair against 25
+// through q_log / q_exp2_prod, and no integer exponent surgery.  The binade table covers 2^-8 <= x < 2^8 (rho2/rho02 of
+// nitromethane stays within [0.3, 3]); the return value says whether x was inside -- outside, the results are finite
+// garbage and the caller must take another route (the sweeps redo the segment with the exact rules, see nmsdt_fused.cu).
+// Relative error <= 3e-16 (table entries and coefficients are rounded long-double values).
+struct PowCoef { double C, D, c[4], d[4]; };       // exponents and binom(C, 2..5), binom(D, 2..5)
+NMSDT_HD bool q_pow_tab(const double* __restrict__ tab, const PowCoef& K, double x, double& xC, double& xD)
+{
+    const int hx = hi_word(x);
+    const int j = (hx >> (20 - LOG_TAB_BITS)) & (LOG_TAB_N - 1);
+    const int e = (hx >> 20) - (1023 + POW_E_MIN);                                      // negative for x < 2^-8, x <= 0, -NaN
+    const int ei = e & (POW_E_N - 1);
+    const double m = mk_double((hx & 0x000fffff) | 0x3ff00000, lo_word(x));            // mantissa in [1,2)
+    const double r = fma(m, tab[IC_OFF + j], -1.0);
+    const double sC = tab[POW_OFF + 2 * j] * tab[PE_OFF + 2 * ei];
+    const double sD = tab[POW_OFF + 2 * j + 1] * tab[PE_OFF + 2 * ei + 1];
+    double qc = fma(r, K.c[3], K.c[2]), qd = fma(r, K.d[3], K.d[2]);
+    qc = fma(r, qc, K.c[1]); qd = fma(r, qd, K.d[1]);
+    qc = fma(r, qc, K.c[0]); qd = fma(r, qd, K.d[0]);
+    qc = fma(r, qc, K.C);    qd = fma(r, qd, K.D);
+    xC = fma(sC * r, qc, sC);
+    xD = fma(sD * r, qd, sD);
+    return (unsigned)e < (unsigned)POW_E_N;
+}
+
+// (x^C, x^D) from one logarithm for arbitrary exponents; C2 = C*log2(e), D2 = D*log2(e).  Needs the ln c_j table.
 NMSDT_HD void q_pow_pair(const double* __restrict__ tab, double x, double C2, double D2, double& xC, double& xD)
 {
     const double L = q_log(tab, x);
@@ -139,16 +172,33 @@ NMSDT_HD double q_exp_neg(const double* __restrict__ tab, double y)
     return q_exp2_prod(tab, cap690(y), -KC[9]);
 }
 
-// host side: fill the 320-double table (long double arithmetic)
-inline void fill_math_tables(double* tab)
+// host side: fill the tables (MATH_TAB_DOUBLES_LOG doubles) and the binomial coefficients for the exponents C, D of
+// Eq. 3-4 (long double arithmetic; the powers use the rounded 1/c_j so that c_j (1 + r) is the mantissa exactly)
+inline void fill_math_tables(double* tab, double C, double D)
 {
     for (int j = 0; j < LOG_TAB_N; ++j) {
         const long double c = 1.0L + ((long double)j + 0.5L) / (long double)LOG_TAB_N;
         const double ic = (double)(1.0L / c);
-        tab[2 * j] = ic;
-        tab[2 * j + 1] = (double)(-logl((long double)ic));
+        const long double cj = 1.0L / (long double)ic;
+        tab[IC_OFF + j] = ic;
+        tab[LC_OFF + j] = (double)logl(cj);
+        tab[POW_OFF + 2 * j] = (double)powl(cj, (long double)C);
+        tab[POW_OFF + 2 * j + 1] = (double)powl(cj, (long double)D);
     }
-    for (int j = 0; j < EXP_TAB_N; ++j) tab[2 * LOG_TAB_N + j] = (double)exp2l((long double)j / (long double)EXP_TAB_N);
+    for (int j = 0; j < EXP_TAB_N; ++j) tab[EXP_OFF + j] = (double)exp2l((long double)j / (long double)EXP_TAB_N);
+    for (int e = 0; e < POW_E_N; ++e) {
+        tab[PE_OFF + 2 * e] = (double)exp2l((long double)(e + POW_E_MIN) * (long double)C);
+        tab[PE_OFF + 2 * e + 1] = (double)exp2l((long double)(e + POW_E_MIN) * (long double)D);
+    }
+}
+inline void fill_pow_coef(PowCoef& K, double C, double D)
+{
+    K.C = C; K.D = D;
+    long double bc = (long double)C, bd = (long double)D;                // binom(a, 1)
+    for (int k = 2; k <= 5; ++k) {
+        bc *= ((long double)C - (k - 1)) / k; bd *= ((long double)D - (k - 1)) / k;
+        K.c[k - 2] = (double)bc; K.d[k - 2] = (double)bd;
+    }
 }
 
 } // namespace nmsdt

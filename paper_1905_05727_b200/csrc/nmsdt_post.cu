@@ -84,8 +84,8 @@ __global__ void __launch_bounds__(HT, 4) k_qdot_hist(const __grid_constant__ Par
                                                   double* __restrict__ part_mass, unsigned long long* __restrict__ count)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
-    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
-    for (int k = threadIdx.x; k < MATH_TAB_DOUBLES; k += HT) s_tab[k] = P.tab[k];
+    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES_LOG];        // with the ln c_j part: Eq. 15 takes a logarithm
+    for (int k = threadIdx.x; k < MATH_TAB_DOUBLES_LOG; k += HT) s_tab[k] = P.tab[k];
     double* s_mass = reinterpret_cast<double*>(s_raw);                         // [HW][nbins]
     int* s_cnt = reinterpret_cast<int*>(s_raw + (size_t)HW * nbins * sizeof(double));   // [HW][nbins]
     for (int k = threadIdx.x; k < HW * nbins; k += HT) { s_mass[k] = 0.0; s_cnt[k] = 0; }

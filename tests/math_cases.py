@@ -43,6 +43,16 @@ def check(probe):
     phys = (xrho > 0.5) & (xrho < 3.0)                        # rho2/rho02 of liquid NM from expansion to the von Neumann spike
     out["powC_phys"], out["powD_phys"] = float(eC[phys].max()), float(eD[phys].max())
     assert out["powC_phys"] <= 1.5e-15 and out["powD_phys"] <= 6e-16, out
+    # the step kernels' route for Eq. 3-4: binade / mantissa tables of c^C, c^D and a binomial series (library powers outside
+    # 2^-8 <= x < 2^8): no condition-number growth
+    yc, yd = probe(7, xrho, C_EXP, D_EXP)
+    out["tabC"] = rel(yc, np.power(xrho.astype(L), L(C_EXP)))
+    out["tabD"] = rel(yd, np.power(xrho.astype(L), L(D_EXP)))
+    assert out["tabC"] <= 4e-16 and out["tabD"] <= 4e-16, out
+    edge = np.array([2.0 ** -8, np.nextafter(2.0 ** -8, 0), np.nextafter(256.0, 0), 256.0, 1.0, np.nextafter(1.0, 0), 0.5, 2.0, 255.99, 0.00391])
+    yc, yd = probe(7, edge, C_EXP, D_EXP)
+    out["tab_edge"] = max(rel(yc, np.power(edge.astype(L), L(C_EXP))), rel(yd, np.power(edge.astype(L), L(D_EXP))))
+    assert out["tab_edge"] <= 4e-16, out
     # exp(-y) = 2^(-y log2 e): the rounding of log2(e) is amplified by y (y = Ta/T2 is 3..40 on this path, Eq. 6)
     y, _ = probe(4, yexp, 0, 0)
     yc = np.minimum(yexp, 690.0)

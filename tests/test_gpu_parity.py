@@ -269,6 +269,38 @@ def test_rare_paths_substepped_source_inside_full_steps(O, B, variant):
         _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="substepped step %d" % it)
 
 
+@pytest.mark.parametrize("patch", [(30, 150, 2.0, 1.0e5), (90, 200, 3.4e5, 1.0e20)])
+def test_rare_paths_density_outside_the_power_tables(O, B, patch):
+    """The fused kernels take x^C, x^D of Eq. 3-4 (x = rho2/rho02) from binade tables that cover 2^-8 <= x < 2^8; a cell or
+    a reconstructed face outside makes the warp redo its segment with the library powers.  A patch of very dilute
+    (x = 1.8e-3) or very dense (x = 300; its pressure is of the size of p_ref(x) ~ 1e20 Pa so that Eq. 2 does not cancel)
+    liquid inside single sweeps of both directions and inside full steps."""
+    cfg = inputs.config("C1", reactive=1)
+    o, s = _pair(O, B, cfg, variant=1)
+    o.init(cfg["init"])
+    o.step(150)
+    q = o.state()
+    e = O.make_eos(cfg["eos"])
+    for (j0, i0, rho2, p) in (patch,):
+        for j in range(j0, j0 + 3):
+            for i in range(i0, i0 + 3):
+                c = O.prim_to_cons(e, np.array([1.2, rho2, 0.0, 0.0, p, 0.3, 1.0]))
+                for k in range(7):
+                    q[k][j, i] = c[k]
+    o.init_fields(q)
+    _sync_state(o, s)
+    dt = 0.2 * o.cfl_dt()
+    for d in (0, 1):
+        o.sweep(d, dt), s.sweep(d, dt)
+        _assert_one_step(o, s, what="sweep %d with densities outside the tables" % d)
+    o.init_fields(q)
+    _sync_state(o, s)
+    for it in range(2):
+        o.step_dt(1, dt), s.step_dt(1, dt)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="step %d with densities outside the tables" % it)
+    assert s.diagnostics()["bad_state"] == 0
+
+
 @pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("d", [0, 1])
 def test_rare_paths_first_order_fallback(O, B, d, variant):
