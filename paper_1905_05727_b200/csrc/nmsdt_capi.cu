@@ -125,6 +125,7 @@ void fill_params(sim* s)
     P.z_min = e.z_min; P.z_max = 1.0 - e.z_min;
     P.C2 = e.C * LOG2E; P.D2 = e.D * LOG2E; P.iG2cv2 = 1.0 / (e.Gamma2 * e.cv2); P.tab = s->tab;
     fill_pow_coef(P.pw, e.C, e.D);
+    P.g1iG1 = e.gamma1 / (e.gamma1 - 1.0);
     P.Ta = k.Ta; P.Cpre = k.Cpre; P.Q = k.Q; P.theta0 = k.substep_theta; P.reactive = k.reactive; P.max_substeps = k.max_substeps;
 }
 

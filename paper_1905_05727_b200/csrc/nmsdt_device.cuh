@@ -28,6 +28,7 @@ struct Params {
     int reactive, max_substeps;
     // fused path (nmsdt_fused.cu): C log2(e), D log2(e), 1/(Gamma2 cv2), device copy of the nmsdt_math.cuh tables
     double C2, D2, iG2cv2;
+    double g1iG1;                // gamma1/(gamma1-1)
     PowCoef pw;                  // exponents C, D of Eq. 3-4 and their binomial coefficients (q_pow_tab)
     const double* tab;
 };

@@ -147,7 +147,7 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     }
     W.p = p; W.lam = lam; W.pr = pr;
     const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
-    const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22) * ixi;  // R10
+    const double rc2 = fma(z1 * P.g1iG1, p, z2 * P.iG2 * r2c22) * ixi;           // R10
     W.rc2 = dmax_(rc2, rho);                                                      // c^2 >= 1
 }
 

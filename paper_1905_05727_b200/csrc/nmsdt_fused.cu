@@ -44,7 +44,7 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     f.rhoE = fma(z1 * P.iG1, p, fma(z2, fma(p - pr, P.iG2, rer), kin));
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
-    const double rc2 = fma(z1 * P.gamma1 * P.iG1, p, z2 * P.iG2 * r2c22);
+    const double rc2 = fma(z1 * P.g1iG1, p, z2 * P.iG2 * r2c22);
     f.c = q_sqrt(floor1(rc2 * q_rcp(xi * rho)));
 }
 
