@@ -237,9 +237,14 @@ constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part
 // the pass is out of place).
 template <int MODE, bool EXACT, int LIM>
 __device__ __forceinline__ bool y_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
-                                          int seg, int col, const double* __restrict__ s_tab, double (*s_q)[7][YT], double (*s_w)[9][YT],
-                                          double (*s_r)[YT], double& smax, int& bad)
+                                          int seg, int col, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad)
 {
+    // thread-private slots, paired so that one 128-bit access moves two values: staged input rows (3 pairs + q6), the
+    // window (W(c-1), 1/rho, rho c^2 and the 7 differences W(c-1) - W(c-2): 8 pairs), the previous right-face state (5 pairs)
+    double2 (*s_q2)[3][YT] = reinterpret_cast<double2 (*)[3][YT]>(s_dyn);
+    double (*s_q1)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + YST * 6 * YT);
+    double2 (*s_w2)[YT] = reinterpret_cast<double2 (*)[YT]>(s_dyn + YST * 7 * YT);
+    double2 (*s_r2)[YT] = reinterpret_cast<double2 (*)[YT]>(s_dyn + (YST * 7 + 16) * YT);
     constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
     const int tid = threadIdx.x;
     bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
@@ -251,9 +256,20 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
     const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
     double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
     const int nrows = c1 - c0 + 4;
-    cp_async8(&s_q[0][0][tid], g); cp_async8(&s_q[0][1][tid], g + fs); cp_async8(&s_q[0][2][tid], g + 3 * fs);
-    cp_async8(&s_q[0][3][tid], g + 2 * fs); cp_async8(&s_q[0][4][tid], g + 4 * fs); cp_async8(&s_q[0][5][tid], g + 5 * fs);
-    cp_async8(&s_q[0][6][tid], g + 6 * fs);
+    auto stage_row = [&](int sg, const double* gp) {      // sweep field order: q0, q1, q3 (normal), q2 (tangential), q4, q5, q6
+        double* d = reinterpret_cast<double*>(&s_q2[sg][0][tid]);
+        cp_async8(d, gp); cp_async8(d + 1, gp + fs);
+        d = reinterpret_cast<double*>(&s_q2[sg][1][tid]);
+        cp_async8(d, gp + 3 * fs); cp_async8(d + 1, gp + 2 * fs);
+        d = reinterpret_cast<double*>(&s_q2[sg][2][tid]);
+        cp_async8(d, gp + 4 * fs); cp_async8(d + 1, gp + 5 * fs);
+        cp_async8(&s_q1[sg][tid], gp + 6 * fs);
+    };
+    auto read_row = [&](int sg, double q[7]) {
+        const double2 a = s_q2[sg][0][tid], b = s_q2[sg][1][tid], c = s_q2[sg][2][tid];
+        q[0] = a.x; q[1] = a.y; q[2] = b.x; q[3] = b.y; q[4] = c.x; q[5] = c.y; q[6] = s_q1[sg][tid];
+    };
+    stage_row(0, g);
     cp_async_commit();
     g += pitch;
     double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
@@ -261,9 +277,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
     for (int jj = 0; jj < nrows; ++jj) {          // row c = c0 - 2 + jj
         const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
         if (jj + 1 < nrows) {
-            cp_async8(&s_q[sn][0][tid], g); cp_async8(&s_q[sn][1][tid], g + fs); cp_async8(&s_q[sn][2][tid], g + 3 * fs);
-            cp_async8(&s_q[sn][3][tid], g + 2 * fs); cp_async8(&s_q[sn][4][tid], g + 4 * fs); cp_async8(&s_q[sn][5][tid], g + 5 * fs);
-            cp_async8(&s_q[sn][6][tid], g + 6 * fs);
+            stage_row(sn, g);
             g += pitch;
         }
         cp_async_commit();
@@ -271,8 +285,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
         FCell Wp;
         {
             double q[7];
-#pragma unroll
-            for (int k = 0; k < 7; ++k) q[k] = s_q[st][k][tid];
+            read_row(st, q);
             double dE, q6n;
             prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n, hot);
         }
@@ -281,28 +294,32 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
         double WL[7], WR[7], lam0c;
         {                                         // centre cell c-1: s_w[0] = W(c-1), s_w[1][0..6] = W(c-1) - W(c-2)
             FCell W0;
-            W0.r1 = s_w[0][0][tid]; W0.r2 = s_w[0][1][tid]; W0.un = s_w[0][2][tid]; W0.ut = s_w[0][3][tid]; W0.p = s_w[0][4][tid];
-            W0.z1 = s_w[0][5][tid]; W0.lam = s_w[0][6][tid]; W0.irho = s_w[0][7][tid]; W0.rc2 = s_w[0][8][tid];
             double a[7];
-#pragma unroll
-            for (int k = 0; k < 7; ++k) a[k] = s_w[1][k][tid];
+            {
+                const double2 w0 = s_w2[0][tid], w1 = s_w2[1][tid], w2 = s_w2[2][tid], w3 = s_w2[3][tid];
+                const double2 w4 = s_w2[4][tid], w5 = s_w2[5][tid], w6 = s_w2[6][tid], w7 = s_w2[7][tid];
+                W0.r1 = w0.x; W0.r2 = w0.y; W0.un = w1.x; W0.ut = w1.y; W0.p = w2.x; W0.z1 = w2.y; W0.lam = w3.x; W0.irho = w3.y;
+                W0.rc2 = w4.x; a[0] = w4.y; a[1] = w5.x; a[2] = w5.y; a[3] = w6.x; a[4] = w6.y; a[5] = w7.x; a[6] = w7.y;
+            }
             const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
             lam0c = W0.lam;
             recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, jj >= 2, hot);      // rows 0, 1: the window is not real yet
-#pragma unroll
-            for (int k = 0; k < 7; ++k) s_w[1][k][tid] = b[k];
+            s_w2[0][tid] = make_double2(Wp.r1, Wp.r2); s_w2[1][tid] = make_double2(Wp.un, Wp.ut); s_w2[2][tid] = make_double2(Wp.p, Wp.z1);
+            s_w2[3][tid] = make_double2(Wp.lam, Wp.irho); s_w2[4][tid] = make_double2(Wp.rc2, b[0]); s_w2[5][tid] = make_double2(b[1], b[2]);
+            s_w2[6][tid] = make_double2(b[3], b[4]); s_w2[7][tid] = make_double2(b[5], b[6]);
         }
-        s_w[0][0][tid] = Wp.r1; s_w[0][1][tid] = Wp.r2; s_w[0][2][tid] = Wp.un; s_w[0][3][tid] = Wp.ut; s_w[0][4][tid] = Wp.p;
-        s_w[0][5][tid] = Wp.z1; s_w[0][6][tid] = Wp.lam; s_w[0][7][tid] = Wp.irho; s_w[0][8][tid] = Wp.rc2;
         FFace fl, fr, pr;
         bool oor = false;                         // a face density outside the power tables (only counted once the window is real)
         face_fast<EXACT>(P, s_tab, WL, fl, oor);
         face_fast<EXACT>(P, s_tab, WR, fr, oor);
         hot |= oor && jj >= 2;
-        pr.r1 = s_r[0][tid]; pr.r2 = s_r[1][tid]; pr.un = s_r[2][tid]; pr.ut = s_r[3][tid]; pr.p = s_r[4][tid];
-        pr.z1 = s_r[5][tid]; pr.lam = s_r[6][tid]; pr.rho = s_r[7][tid]; pr.rhoE = s_r[8][tid]; pr.c = s_r[9][tid];
-        s_r[0][tid] = fr.r1; s_r[1][tid] = fr.r2; s_r[2][tid] = fr.un; s_r[3][tid] = fr.ut; s_r[4][tid] = fr.p;
-        s_r[5][tid] = fr.z1; s_r[6][tid] = fr.lam; s_r[7][tid] = fr.rho; s_r[8][tid] = fr.rhoE; s_r[9][tid] = fr.c;
+        {
+            const double2 r0 = s_r2[0][tid], r1 = s_r2[1][tid], r2 = s_r2[2][tid], r3 = s_r2[3][tid], r4 = s_r2[4][tid];
+            pr.r1 = r0.x; pr.r2 = r0.y; pr.un = r1.x; pr.ut = r1.y; pr.p = r2.x; pr.z1 = r2.y; pr.lam = r3.x; pr.rho = r3.y;
+            pr.rhoE = r4.x; pr.c = r4.y;
+        }
+        s_r2[0][tid] = make_double2(fr.r1, fr.r2); s_r2[1][tid] = make_double2(fr.un, fr.ut); s_r2[2][tid] = make_double2(fr.p, fr.z1);
+        s_r2[3][tid] = make_double2(fr.lam, fr.rho); s_r2[4][tid] = make_double2(fr.rhoE, fr.c);
         double F[8];
         hllc_fast(pr, fl, F);                     // face between cells c-2 and c-1
         {                                         // finish cell c-2
@@ -327,8 +344,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
         }
         {                                         // start cell c-1 with its lower-face flux
             double o[7];
-#pragma unroll
-            for (int k = 0; k < 7; ++k) o[k] = s_q[sp][k][tid];
+            read_row(sp, o);
             if (MODE == MODE_LEAD) lead_fix(P, o, lam0c);
             z1n = o[5];
 #pragma unroll
@@ -347,18 +363,15 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
 {
     extern __shared__ __align__(16) double s_dyn[];
     __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];     // static: table lookups address it as [idx + const]
-    double (*s_q)[7][YT] = reinterpret_cast<double (*)[7][YT]>(s_dyn);
-    double (*s_w)[9][YT] = reinterpret_cast<double (*)[9][YT]>(s_dyn + YST * 7 * YT);
-    double (*s_r)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + (YST * 7 + 9 + 7) * YT);
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
     const int col = blockIdx.x * YT + threadIdx.x;
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
-        const bool redo = y_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+        const bool redo = y_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_dyn, smax, bad);
         if (__any_sync(__activemask(), redo)) {                  // rare: redo the warp's segment with the exact R13 / R17 rules
             smax = 0.0; bad = 0;
-            y_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_q, s_w, s_r, smax, bad);
+            y_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_dyn, smax, bad);
         }
     }
     if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
@@ -378,9 +391,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
     constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
     double* s_ring = s_dyn;
     bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
-    double* rw = s_ring + warp * RING_DOUBLES;       // [16][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
-    double* rfr = rw + 16 * RING;                    // [10][33]: right-face state of cell A
-    double* rf = rfr + 10 * RING;                    // [8][33] : flux of face A-1/2
+    // rings of value PAIRS (one 128-bit access moves two values)
+    double2* rw = reinterpret_cast<double2*>(s_ring + warp * RING_DOUBLES);   // [8][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
+    double2* rfr = rw + 8 * RING;                    // [5][33]: right-face state of cell A
+    double2* rf = rfr + 5 * RING;                    // [4][33]: flux of face A-1/2
     double2* stg = reinterpret_cast<double2*>(s_dyn + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
     const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
@@ -425,11 +439,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
             prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n, hotb);
             hot |= hotb && Ac <= P.nx;
-            rw[0 * RING + sw] = WA.r1; rw[1 * RING + sw] = WA.r2; rw[2 * RING + sw] = WA.un; rw[3 * RING + sw] = WA.ut;
-            rw[4 * RING + sw] = WA.p;  rw[5 * RING + sw] = WA.z1; rw[6 * RING + sw] = WA.lam;
-            rw[7 * RING + sw] = WB.r1; rw[8 * RING + sw] = WB.r2; rw[9 * RING + sw] = WB.un; rw[10 * RING + sw] = WB.ut;
-            rw[11 * RING + sw] = WB.p; rw[12 * RING + sw] = WB.z1; rw[13 * RING + sw] = WB.lam;
-            rw[14 * RING + sw] = WB.irho; rw[15 * RING + sw] = WB.rc2;
+            rw[0 * RING + sw] = make_double2(WA.r1, WA.r2); rw[1 * RING + sw] = make_double2(WA.un, WA.ut);
+            rw[2 * RING + sw] = make_double2(WA.p, WA.z1);  rw[3 * RING + sw] = make_double2(WA.lam, WB.r1);
+            rw[4 * RING + sw] = make_double2(WB.r2, WB.un); rw[5 * RING + sw] = make_double2(WB.ut, WB.p);
+            rw[6 * RING + sw] = make_double2(WB.z1, WB.lam); rw[7 * RING + sw] = make_double2(WB.irho, WB.rc2);
         }
         __syncwarp();
         // ---- phase 2: reconstruct cells A-1 and A, four face states ------------------------------------------
@@ -437,11 +450,14 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         double lam_u0 = 0.0, lam_u1 = 0.0;
         {
             FCell Wmm, Wm1;
-            Wmm.r1 = rw[0 * RING + sr]; Wmm.r2 = rw[1 * RING + sr]; Wmm.un = rw[2 * RING + sr]; Wmm.ut = rw[3 * RING + sr];
-            Wmm.p = rw[4 * RING + sr];  Wmm.z1 = rw[5 * RING + sr]; Wmm.lam = rw[6 * RING + sr]; Wmm.irho = 0.0; Wmm.rc2 = 0.0;
-            Wm1.r1 = rw[7 * RING + sr]; Wm1.r2 = rw[8 * RING + sr]; Wm1.un = rw[9 * RING + sr]; Wm1.ut = rw[10 * RING + sr];
-            Wm1.p = rw[11 * RING + sr]; Wm1.z1 = rw[12 * RING + sr]; Wm1.lam = rw[13 * RING + sr];
-            Wm1.irho = rw[14 * RING + sr]; Wm1.rc2 = rw[15 * RING + sr];
+            {
+                const double2 v0 = rw[0 * RING + sr], v1 = rw[1 * RING + sr], v2 = rw[2 * RING + sr], v3 = rw[3 * RING + sr];
+                const double2 v4 = rw[4 * RING + sr], v5 = rw[5 * RING + sr], v6 = rw[6 * RING + sr], v7 = rw[7 * RING + sr];
+                Wmm.r1 = v0.x; Wmm.r2 = v0.y; Wmm.un = v1.x; Wmm.ut = v1.y; Wmm.p = v2.x; Wmm.z1 = v2.y; Wmm.lam = v3.x;
+                Wmm.irho = 0.0; Wmm.rc2 = 0.0;
+                Wm1.r1 = v3.y; Wm1.r2 = v4.x; Wm1.un = v4.y; Wm1.ut = v5.x; Wm1.p = v5.y; Wm1.z1 = v6.x; Wm1.lam = v6.y;
+                Wm1.irho = v7.x; Wm1.rc2 = v7.y;
+            }
             lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
             double WL[7], WR[7];
             bool oor = false;                        // a face density outside the power tables
@@ -453,22 +469,25 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             FFace FR2;
             face_fast<EXACT>(P, s_tab, WR, FR2, oor);
             hot |= oor && (k > 0 || lane > 0);
-            rfr[0 * RING + sw] = FR2.r1; rfr[1 * RING + sw] = FR2.r2; rfr[2 * RING + sw] = FR2.un; rfr[3 * RING + sw] = FR2.ut;
-            rfr[4 * RING + sw] = FR2.p;  rfr[5 * RING + sw] = FR2.z1; rfr[6 * RING + sw] = FR2.lam; rfr[7 * RING + sw] = FR2.rho;
-            rfr[8 * RING + sw] = FR2.rhoE; rfr[9 * RING + sw] = FR2.c;
+            rfr[0 * RING + sw] = make_double2(FR2.r1, FR2.r2); rfr[1 * RING + sw] = make_double2(FR2.un, FR2.ut);
+            rfr[2 * RING + sw] = make_double2(FR2.p, FR2.z1);  rfr[3 * RING + sw] = make_double2(FR2.lam, FR2.rho);
+            rfr[4 * RING + sw] = make_double2(FR2.rhoE, FR2.c);
         }
         __syncwarp();
         // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
         double F1[8], F2[8];
         {
             FFace FRp;
-            FRp.r1 = rfr[0 * RING + sr]; FRp.r2 = rfr[1 * RING + sr]; FRp.un = rfr[2 * RING + sr]; FRp.ut = rfr[3 * RING + sr];
-            FRp.p = rfr[4 * RING + sr];  FRp.z1 = rfr[5 * RING + sr]; FRp.lam = rfr[6 * RING + sr]; FRp.rho = rfr[7 * RING + sr];
-            FRp.rhoE = rfr[8 * RING + sr]; FRp.c = rfr[9 * RING + sr];
+            {
+                const double2 v0 = rfr[0 * RING + sr], v1 = rfr[1 * RING + sr], v2 = rfr[2 * RING + sr], v3 = rfr[3 * RING + sr];
+                const double2 v4 = rfr[4 * RING + sr];
+                FRp.r1 = v0.x; FRp.r2 = v0.y; FRp.un = v1.x; FRp.ut = v1.y; FRp.p = v2.x; FRp.z1 = v2.y; FRp.lam = v3.x; FRp.rho = v3.y;
+                FRp.rhoE = v4.x; FRp.c = v4.y;
+            }
             hllc_fast(FRp, FL1, F1);
             hllc_fast(FR1, FL2, F2);
 #pragma unroll
-            for (int f = 0; f < 8; ++f) rf[f * RING + sw] = F2[f];
+            for (int f = 0; f < 4; ++f) rf[f * RING + sw] = make_double2(F2[2 * f], F2[2 * f + 1]);
         }
         __syncwarp();
         // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
@@ -477,7 +496,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             const bool valid = k > 0 && u0 < c1;
             double F0[8];
 #pragma unroll
-            for (int f = 0; f < 8; ++f) F0[f] = rf[f * RING + sr];
+            for (int f = 0; f < 4; ++f) { const double2 v = rf[f * RING + sr]; F0[2 * f] = v.x; F0[2 * f + 1] = v.y; }
             const int pl = ps == 0 ? PRING - 1 : ps - 1;      // the pair staged by the left neighbour = cells u0, u0+1
             double oa[7], ob[7];
 #pragma unroll
