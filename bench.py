@@ -151,7 +151,7 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
-def run_slab(args, torch, dist, binding, rank, world, local):
+def run_slab(args, torch, dist, binding, rank, world, local, shared_gpu=False):
     """one domain of `world` x the workload's columns, one x-slab per rank (weak scaling; DistSlab)"""
     from paper_1905_05727_b200 import slab
     K, Wm = max(1, args.steps), max(3, args.warmup)
@@ -189,7 +189,8 @@ def run_slab(args, torch, dist, binding, rank, world, local):
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "%s x %d along x: one domain %dx%d cut into %d x-slabs, halo transport %s, dt by max-allreduce"
                                    % (args.config, world, g["nx"], g["ny"], world, args.transport),
-                       "parallelism": "x-slabs", "l2_policy": "inputs larger than L2"},
+                       "parallelism": "x-slabs", "l2_policy": "inputs larger than L2",
+                       "ranks_share_a_gpu": bool(shared_gpu)},          # true = plumbing check on a one-GPU box, not a measurement
             "clocks": sampler.summary(), "e2e": None, "gpu_launches": int(launches),
             "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "M2r": d["M2r"]}}))
     ds.close()
@@ -222,12 +223,17 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    # one rank per GPU over NCCL.  When the node has fewer GPUs than local ranks (a one-GPU box running the plumbing check of
+    # tests/test_gpu_slab.py), the ranks share devices and gloo carries the collectives: NCCL refuses two ranks on one GPU.
+    ndev = torch.cuda.device_count()
+    shared_gpu = world > 1 and int(os.environ.get("LOCAL_WORLD_SIZE", str(world))) > ndev
+    local = local % ndev
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl")
+        dist.init_process_group("gloo" if shared_gpu else "nccl")
     K, Wm = max(1, args.steps), max(3, args.warmup)
     if args.decomp == "slab" and world > 1:
-        return run_slab(args, torch, dist, binding, rank, world, local)
+        return run_slab(args, torch, dist, binding, rank, world, local, shared_gpu)
 
     cfg = inputs.config(args.config, seed=inputs.config(args.config)["init"]["seed"] + rank if args.config in ("C4", "C5") else None)
     g = cfg["grid"]

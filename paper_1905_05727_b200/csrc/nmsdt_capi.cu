@@ -126,6 +126,9 @@ void fill_params(sim* s)
     P.C2 = e.C * LOG2E; P.D2 = e.D * LOG2E; P.iG2cv2 = 1.0 / (e.Gamma2 * e.cv2); P.tab = s->tab;
     fill_pow_coef(P.pw, e.C, e.D);
     P.g1iG1 = e.gamma1 / (e.gamma1 - 1.0);
+    // rho2 e_ref2 - p_ref2/Gamma2 = E1 x^C + E2 x^D - E3 x and rho2 c2^2 - (Gamma2+1) p = R1 x^C + R2 x^D  (Eq. 3-4 in O2)
+    P.E1 = P.kA - e.A / e.Gamma2; P.E2 = P.kB + e.B / e.Gamma2; P.E3 = P.kA + P.kB;
+    P.R1 = e.A * (e.C - (e.Gamma2 + 1.0)); P.R2 = e.B * ((e.Gamma2 + 1.0) - e.D);
     P.Ta = k.Ta; P.Cpre = k.Cpre; P.Q = k.Q; P.theta0 = k.substep_theta; P.reactive = k.reactive; P.max_substeps = k.max_substeps;
 }
 

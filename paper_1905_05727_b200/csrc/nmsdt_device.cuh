@@ -29,6 +29,7 @@ struct Params {
     // fused path (nmsdt_fused.cu): C log2(e), D log2(e), 1/(Gamma2 cv2), device copy of the nmsdt_math.cuh tables
     double C2, D2, iG2cv2;
     double g1iG1;                // gamma1/(gamma1-1)
+    double E1, E2, E3, R1, R2;   // Eq. 3-4 folded into the closure: see face_fast / prim_cell
     PowCoef pw;                  // exponents C, D of Eq. 3-4 and their binomial coefficients (q_pow_tab)
     const double* tab;
 };

@@ -125,15 +125,16 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     W.z1 = z1;
     W.r1 = q[0] * q_rcp(z1);
     W.r2 = q[1] * q_rcp(z2);
-    const double rhoe = fma(-0.5 * irho, fma(q[2], q[2], q[3] * q[3]), q[4]);
+    const double rhoe = fma(-0.5, fma(q[2], W.un, q[3] * W.ut), q[4]);
     const double x = W.r2 * P.irho02;
     double xC, xD;
     eos_pow<EX>(P, tab, x, xC, xD, hot);
-    const double pr = fma(P.A, xC, -P.B * xD);                                   // Eq. 3
-    const double rer = fma(P.kA, xC - x, P.kB * (xD - x));                       // rho2 * Eq. 4
+    const double pr = fma(P.A, xC, -P.B * xD);                                   // Eq. 3 (dead code unless T2 is wanted)
+    // rho2 e_ref2 - p_ref2/Gamma2 = E1 x^C + E2 x^D - E3 x  (Eq. 3-4 folded, O2)
+    const double gx = fma(P.E1, xC, fma(P.E2, xD, -P.E3 * x));
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double ixi = q_rcp(xi);
-    double p = (rhoe - z2 * fma(-pr, P.iG2, rer)) * ixi;
+    double p = fma(-z2, gx, rhoe) * ixi;
     double lam = clamp01(q[6] * iq1);
     dE = 0.0; q6n = q[6];
     if (SRC != SRC_NONE) {
@@ -146,7 +147,7 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
         lam = lam1;
     }
     W.p = p; W.lam = lam; W.pr = pr;
-    const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
+    const double r2c22 = fma(P.R1, xC, fma(P.R2, xD, P.G2p1 * p));               // rho2 c2^2
     const double rc2 = fma(z1 * P.g1iG1, p, z2 * P.iG2 * r2c22) * ixi;           // R10
     W.rc2 = dmax_(rc2, rho);                                                      // c^2 >= 1
 }

@@ -38,12 +38,13 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     const double x = W[1] * P.irho02;
     double xC, xD;
     eos_pow<EX>(P, tab, x, xC, xD, oor);
-    const double pr = fma(P.A, xC, -P.B * xD);
-    const double rer = fma(P.kA, xC - x, P.kB * (xD - x));
+    // Eq. 3-4 enter the closure only through two fixed combinations of x^C, x^D, x (O2):
+    //   (p - p_ref2)/Gamma2 + rho2 e_ref2 = p/Gamma2 + E1 x^C + E2 x^D - E3 x,   rho2 c2^2 = (Gamma2+1) p + R1 x^C + R2 x^D
+    const double brk = fma(p, P.iG2, fma(P.E1, xC, fma(P.E2, xD, -P.E3 * x)));
     const double kin = 0.5 * rho * fma(W[2], W[2], W[3] * W[3]);
-    f.rhoE = fma(z1 * P.iG1, p, fma(z2, fma(p - pr, P.iG2, rer), kin));
+    f.rhoE = fma(z1 * P.iG1, p, fma(z2, brk, kin));
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
-    const double r2c22 = fma(P.G2p1, p - pr, fma(P.AC, xC, -P.BD * xD));
+    const double r2c22 = fma(P.R1, xC, fma(P.R2, xD, P.G2p1 * p));
     const double rc2 = fma(z1 * P.g1iG1, p, z2 * P.iG2 * r2c22);
     f.c = q_sqrt(floor1(rc2 * q_rcp(xi * rho)));
 }
@@ -76,13 +77,13 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
     double D[7];
 #pragma unroll
     for (int k = 0; k < 7; ++k) D[k] = limited_f<LIM>(a[k], b[k]);
-    const double u = W0.un;
-    {
-        const double m0 = fma(-khalf, fma(u, D[0], W0.r1 * D[2]), w0[0]);
-        const double m1 = fma(-khalf, fma(u, D[1], W0.r2 * D[2]), w0[1]);
-        WL[0] = fma(-0.5, D[0], m0); WR[0] = fma(0.5, D[0], m0);
-        WL[1] = fma(-0.5, D[1], m1); WR[1] = fma(0.5, D[1], m1);
-    }
+    // predictor W - k (u D + coupling terms) (O4.2), written so that every component is a chain of fma on k u, k D_u, k D_p
+    const double ku = khalf * W0.un;
+    const double kDu = khalf * D[2];
+    const double m0 = fma(-ku, D[0], fma(-kDu, W0.r1, w0[0]));
+    const double m1 = fma(-ku, D[1], fma(-kDu, W0.r2, w0[1]));
+    WL[0] = fma(-0.5, D[0], m0); WR[0] = fma(0.5, D[0], m0);
+    WL[1] = fma(-0.5, D[1], m1); WR[1] = fma(0.5, D[1], m1);
     // all four > 0 (a positive subnormal counts as zero)
     const bool ok = min(min(hi_word(WL[0]), hi_word(WL[1])), min(hi_word(WR[0]), hi_word(WR[1]))) > 0;
     if (EXACT) {
@@ -93,17 +94,18 @@ __device__ __forceinline__ void recon_core(const Params& P, const FCell& W0, con
     } else {
         redo |= counted && !ok;
     }
-    double d[7];
-    d[2] = fma(u, D[2], D[4] * W0.irho);
-    d[3] = u * D[3];
-    d[4] = fma(u, D[4], W0.rc2 * D[2]);
-    d[5] = u * D[5];
-    d[6] = u * D[6];
+    // (EXACT with a fallback cell: every D[k] is zero from here on and the densities above were replaced, so k Du = 0 too)
+    const double kDu2 = khalf * D[2], kDp = khalf * D[4];
+    double m[7];
+    m[2] = fma(-ku, D[2], fma(-kDp, W0.irho, w0[2]));
+    m[3] = fma(-ku, D[3], w0[3]);
+    m[4] = fma(-ku, D[4], fma(-kDu2, W0.rc2, w0[4]));
+    m[5] = fma(-ku, D[5], w0[5]);
+    m[6] = fma(-ku, D[6], w0[6]);
 #pragma unroll
     for (int k = 2; k < 7; ++k) {
-        const double m = fma(-khalf, d[k], w0[k]);
-        WL[k] = fma(-0.5, D[k], m);
-        WR[k] = fma(0.5, D[k], m);
+        WL[k] = fma(-0.5, D[k], m[k]);
+        WR[k] = fma(0.5, D[k], m[k]);
     }
 }
 

@@ -198,3 +198,31 @@ def test_distslab_two_processes_on_one_gpu(B, tmp_path, transport, port):
     d = one.diagnostics()
     for p in parts:
         assert float(p["t"]) == d["t"] and float(p["M2r"]) == pytest.approx(d["M2r"], rel=1e-12)
+
+
+@pytest.mark.parametrize("transport,port", [("staged", 29641), ("peer", 29642)])
+def test_bench_decomp_slab_two_ranks_on_one_gpu(B, transport, port):
+    """`bench.py --decomp slab` under torchrun, as the driver would launch it for N = 2, on the one GPU there is (the ranks
+    share it and gloo carries the collectives: a plumbing check, not a measurement): one JSON line from rank 0, a domain of
+    2 x C3's columns advanced by both ranks to the same step, finite state."""
+    import json
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="2")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+                        "127.0.0.1", "--master-port", str(port), "bench.py", "--gpus", "2", "--steps", "4", "--warmup", "3",
+                        "--config", "C3", "--decomp", "slab", "--transport", transport],
+                       capture_output=True, text=True, cwd=ROOT, env=env, timeout=900)
+    assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["config"]["parallelism"] == "x-slabs" and d["config"]["ranks_share_a_gpu"] is True
+    assert d["sim"]["step"] == 7 and d["sim"]["bad_state"] == 0 and d["value"] > 0 and d["gpu_launches"] > 0
+    # the same domain undivided, same number of steps: identical clock and (up to summation order) identical reactive mass
+    cfg = inputs.config("C3")
+    g = dict(cfg["grid"], nx=2 * cfg["grid"]["nx"])
+    ini = dict(cfg["init"], x_hi=g["nx"])
+    one = B.Sim(g, cfg["eos"], cfg["kin"])
+    one.init(ini)
+    one.step(7)
+    d1 = one.diagnostics()
+    assert d["sim"]["t"] == d1["t"] and d["sim"]["M2r"] == pytest.approx(d1["M2r"], rel=1e-12)
