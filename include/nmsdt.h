@@ -226,6 +226,7 @@ int sim_probe_fp64(sim_t*, double* gflops_out, double* ms_out);
      0: 1/x            1: sqrt(x)        2: ln(x)        3: (x^a, x^b)        4: exp(-x)
      5: (max(x,1), min(max(x,0),1))      6: (max(x,0), min(x,690))
      7: (x^C, x^D) for the handle's own Eq. 3 exponents by the table route of the step kernels (a, b ignored)
+     8: (max(sqrt(x/a), 1), max(sqrt(a/x), 1)): the floored sound speed of R10 from rho c^2 and rho without a reciprocal
    x must be a positive normal number for 0-3. SIM_ERR_ARG on NULL / n < 1 / unknown fn. [sync] */
 int sim_probe_math(sim_t*, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1);
 

@@ -810,7 +810,7 @@ int sim_shock_kinematics(sim_t* s, const double* host_t, const double* host_xs, 
 
 int sim_probe_math(sim_t* s, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1)
 {
-    if (!s || !host_x || !host_y0 || !host_y1 || n < 1 || fn < 0 || fn > 7) return fail(s, SIM_ERR_ARG, "sim_probe_math: bad argument");
+    if (!s || !host_x || !host_y0 || !host_y1 || n < 1 || fn < 0 || fn > 8) return fail(s, SIM_ERR_ARG, "sim_probe_math: bad argument");
     if (launch_probe_math(s->P.pw, s->P.tab, fn, host_x, n, a, b, host_y0, host_y1, s->stream)) return fail(s, SIM_ERR_CUDA, "sim_probe_math failed");
     s->launches += 1;
     return SIM_OK;

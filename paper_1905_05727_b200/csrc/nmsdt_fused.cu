@@ -46,7 +46,7 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double r2c22 = fma(P.R1, xC, fma(P.R2, xD, P.G2p1 * p));
     const double rc2 = fma(z1 * P.g1iG1, p, z2 * P.iG2 * r2c22);
-    f.c = q_sqrt(floor1(rc2 * q_rcp(xi * rho)));
+    f.c = q_sqrt_ratio_floor1(rc2, xi * rho);            // c = sqrt(max(rho c^2 / rho, 1)) (R10)
 }
 
 template <int LIM>
@@ -154,12 +154,16 @@ __device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double
     F[7] = uf;
 }
 
-__device__ __forceinline__ bool all_finite7(const double o[7])
+// state check of a finished cell on the high words (integer pipe): q0, q1 positive normal numbers, q2, q3, q4, q6 and the
+// wavespeed finite.  (q5 was clamped just before and cannot be non-finite here.)
+__device__ __forceinline__ bool state_ok(const double o[7], double a)
 {
-    int m = 0;
-#pragma unroll
-    for (int k = 0; k < 7; ++k) m = max(m, __double2hiint(o[k]) & 0x7fffffff);
-    return m < 0x7ff00000;
+    const int pos = min(__double2hiint(o[0]), __double2hiint(o[1]));
+    int m = max(__double2hiint(o[0]), __double2hiint(o[1]));
+    m = max(m, max(__double2hiint(o[2]) & 0x7fffffff, __double2hiint(o[3]) & 0x7fffffff));
+    m = max(m, max(__double2hiint(o[4]) & 0x7fffffff, __double2hiint(o[6]) & 0x7fffffff));
+    m = max(m, __double2hiint(a) & 0x7fffffff);
+    return pos > 0 && m < 0x7ff00000;
 }
 
 // finished cell of the second pass: trailing S(dt/2) (SRC != SRC_NONE), wavespeed of the new state, state check (a6, a7, R17)
@@ -171,8 +175,7 @@ __device__ __forceinline__ void trail_cell(const Params& P, const double* __rest
     prim_cell<SRC, EX>(P, tab, o, tau, Tsafe, W, dE, q6n, hot);
     o[4] += dE; o[6] = q6n;
     const double a = dmax_(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
-    const bool ok = all_finite7(o) && o[0] > 0.0 && o[1] > 0.0 && (__double2hiint(a) & 0x7fffffff) < 0x7ff00000;
-    bad |= ok ? 0 : 1;
+    bad |= state_ok(o, a) ? 0 : 1;
     smax = dmax_(smax, a);
 }
 
@@ -735,6 +738,7 @@ __global__ void __launch_bounds__(128) k_probe_math(const __grid_constant__ PowC
     case 4: r0 = q_exp_neg(s_tab, v); break;
     case 5: r0 = floor1(v); r1 = clamp01(v); break;
     case 6: r0 = nonneg(v); r1 = cap690(v); break;
+    case 8: r0 = q_sqrt_ratio_floor1(v, a); r1 = q_sqrt_ratio_floor1(a, v); break;   // max(sqrt(x/a), 1), max(sqrt(a/x), 1)
     case 7: if (!q_pow_tab(s_tab, pw, v, r0, r1)) { r0 = pow(v, pw.C); r1 = pow(v, pw.D); } break;   // the step kernels' route for Eq. 3-4
     default: break;
     }

@@ -85,6 +85,21 @@ NMSDT_HD double q_sqrt(double x)
     return fma(t, p, t);
 }
 
+// max(sqrt(n/d), 1) for d > 0 without a reciprocal: sqrt(n/d) = n rsqrt(n d), the reciprocal square root refined as in
+// q_sqrt (seed y ~ (1+delta)/sqrt(x), e = 1 - x y^2, y (1 + e/2 + 3 e^2/8)): 7 FP64 instructions instead of the 9 of
+// q_sqrt(n * q_rcp(d)), one MUFU instead of two.  n <= 0 (the c >= 1 m/s floor of R10 in strongly expanded liquid), NaN and
+// overflow all give 1: one unsigned range test on the high word lets only results in [1, inf) through.
+NMSDT_HD double q_sqrt_ratio_floor1(double n, double d)
+{
+    const double x = n * d;
+    const double y = rsq_seed(x);
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(e, 0.375, 0.5) * e;
+    const double c = n * fma(y, p, y);
+    return (unsigned)(hi_word(c) - 0x3ff00000) < 0x40000000u ? c : 1.0;
+}
+
 // Clamps decided on the high word (integer pipe instead of the FP64 pipe).  For finite x:
 //   floor1(x)  = max(x, 1)      (x < 1, zero or negative -> 1; the signed compare sends negative x below 0x3ff00000)
 //   clamp01(x) = min(max(x, 0), 1)

@@ -53,6 +53,14 @@ def check(probe):
     yc, yd = probe(7, edge, C_EXP, D_EXP)
     out["tab_edge"] = max(rel(yc, np.power(edge.astype(L), L(C_EXP))), rel(yd, np.power(edge.astype(L), L(D_EXP))))
     assert out["tab_edge"] <= 4e-16, out
+    # floored sound speed max(sqrt(n/d), 1) by the refined reciprocal square root of n d (n <= 0 -> 1)
+    dd = 1134.0 * 0.84
+    nn = np.concatenate([pos[(pos > 1e-6) & (pos < 1e12)] * dd, [dd, dd * (1 + 1e-15), dd * (1 - 1e-15), 0.0, -5.0, -1e300]])
+    y0, y1 = probe(8, nn, dd, 0)
+    ref = np.maximum(np.sqrt(np.maximum(nn, 0).astype(L) / L(dd)), 1)
+    out["sqrt_ratio"] = rel(y0, ref)
+    assert out["sqrt_ratio"] <= 5e-16, out
+    assert np.all(y0 >= 1.0) and np.all(y0[-3:] == 1.0) and np.all(np.isfinite(y1[:-3])) and np.all(y1[-3:] == 1.0)
     # exp(-y) = 2^(-y log2 e): the rounding of log2(e) is amplified by y (y = Ta/T2 is 3..40 on this path, Eq. 6)
     y, _ = probe(4, yexp, 0, 0)
     yc = np.minimum(yexp, 690.0)

@@ -26,6 +26,7 @@ extern "C" int math_probe(int fn, const double* x, int n, double a, double b, do
         case 4: r0 = q_exp_neg(tab, v); break;
         case 5: r0 = floor1(v); r1 = clamp01(v); break;
         case 6: r0 = nonneg(v); r1 = cap690(v); break;
+        case 8: r0 = q_sqrt_ratio_floor1(v, a); r1 = q_sqrt_ratio_floor1(a, v); break;
         case 7: if (!q_pow_tab(tab, pw, v, r0, r1)) { r0 = pow(v, pw.C); r1 = pow(v, pw.D); } break;
         default: return -1;
         }
