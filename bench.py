@@ -37,12 +37,12 @@ UNIT = "cell-updates/s"
 # C5 launches (profiles/r01h_fused_c5.md) divided by the ramp-up redundancy of a segment (65/64 on C5).
 #   FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot):
 FP64_INSTR_PER_CELL = {"lead": 352.0, "trail": 417.0}       # pass 1 = S + sweep; pass 2 = sweep + S + wavespeed
-#   flops with dadd = dmul = 1, dfma = 2 (52 % of the FP64 instructions are DFMA):
-FLOP_PER_CELL = {"lead": 553.0, "trail": 654.0}
+#   flops with dadd = dmul = 1, dfma = 2, dsetp = 0 (54 % of the FP64 instructions are DFMA):
+FLOP_PER_CELL = {"lead": 524.0, "trail": 617.0}
 FP64_LANES_PER_SM, N_SM = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per cell per launch from the ncu --set full capture of C5 (mean of the
 # lead and trail launches; profiles/r01h_fused_c5.md): 113.0 B (x), 112.6 B (y) against 112 B algorithmic
-TRAFFIC_BYTES_PER_CELL = {"sweep_x": 113.0, "sweep_y": 112.6}
+TRAFFIC_BYTES_PER_CELL = {"sweep_x": 112.95, "sweep_y": 112.6}
 
 
 def peaks():
