@@ -111,7 +111,8 @@ const char* sim_last_error(const sim_t*);          /* sim may be NULL: error of 
 /* Initial condition on the device: cavity placement (generator R16 runs on the GPU), tanh painting,
    ambient state and shocked slab (O7).  Resets t, step; computes M2,tot and the first CFL dt. [sync] */
 int sim_init(sim_t*, const sim_init_t*);
-/* Explicit initial state from 7 HOST arrays of nx*ny doubles (row-major, x fastest). [sync] */
+/* Explicit initial state from 7 HOST arrays of nx*ny doubles (row-major, x fastest).  q5 is clamped to
+   [z_min, 1 - z_min] on entry (O3's clamp; a state the scheme produced is already inside and is stored unchanged). [sync] */
 int sim_init_fields(sim_t*, const double* const host_q[7]);
 
 /* CFL time step of the current state (a7). [sync] */

@@ -389,6 +389,8 @@ int sim_init_fields(sim_t* s, const double* const host_q[7])
         if (cudaMemcpy2DAsync(dst, (size_t)P.pitch * 8, host_q[f], (size_t)P.nx * 8, (size_t)P.nx * 8, P.ny, cudaMemcpyHostToDevice, s->stream) != cudaSuccess)
             return check_cuda(s, "sim_init_fields");
     }
+    launch_clamp_z1(P, s->A + 5 * P.fstride, s->stream);       // q5 within [z_min, 1 - z_min]: the invariant of every stored state
+    s->launches++;
     cudaStreamSynchronize(s->stream);
     if (s->d_cav) { cudaFree(s->d_cav); s->d_cav = nullptr; }
     s->ncav = 0;

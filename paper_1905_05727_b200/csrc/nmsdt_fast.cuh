@@ -106,7 +106,8 @@ __device__ __forceinline__ void eos_pow(const Params& P, const double* __restric
     }
 }
 
-// O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.
+// O3 (+ O5 when SRC): conserved (normal / tangential momentum ordered) -> primitives.  O3's clamp of z1 is an invariant of
+// the stored q5 here (O4.6 clamps every updated cell; sim_init / sim_init_fields clamp what they write), not a step.
 // SRC: the Arrhenius step over tau is applied to the cell; dE = energy moved into rho E, q6n = new z2 rho2 lambda.
 // The kernels that apply the source are only launched for reactive runs (launch_sweep_fused), so there is no
 // P.reactive test here.
@@ -119,7 +120,7 @@ __device__ __forceinline__ void prim_cell(const Params& P, const double* __restr
     W.irho = irho;
     W.un = q[2] * irho;
     W.ut = q[3] * irho;
-    const double z1 = clampf(q[5], P.z_min, P.z_max);
+    const double z1 = q[5];          // within [z_min, 1 - z_min] for every state in HBM: clamped on store by the sweeps and by sim_init*
     const double z2 = 1.0 - z1;
     const double iq1 = q_rcp(q[1]);
     W.z1 = z1;

@@ -56,6 +56,7 @@ void launch_slab_move(const SlabView& src, const SlabView& dst, int ny, cudaStre
 
 // init / output kernels (nmsdt_init.cu)
 void launch_zero_plane(const Params& P, double* plane, cudaStream_t s);
+void launch_clamp_z1(const Params& P, double* q5, cudaStream_t s);
 void launch_shift_cavities(Cav* cav, int n, double shift, cudaStream_t s);
 void launch_paint(const Params& P, double* prof_plane, const Cav* cav, int ncav, double h, cudaStream_t s);
 void launch_fill_state(const Params& P, double* q, int shock_cells, Hug hug, double p_shock, double p0, double rho1_0,

@@ -49,6 +49,22 @@ void launch_paint(const Params& P, double* prof, const Cav* cav, int ncav, doubl
     if (ncav > 0) k_paint<<<ncav, 256, 0, s>>>(P, prof, cav, ncav, h);
 }
 
+// explicit initial states (sim_init_fields): q5 into [z_min, 1 - z_min], the invariant the fused kernels' primitive recovery
+// relies on (O3 clamps at every recovery; an in-range q5, which is all the scheme ever produces, is unchanged)
+__global__ void k_clamp_z1(const __grid_constant__ Params P, double* __restrict__ q5)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.nx) return;
+    double* p = q5 + (long long)(blockIdx.y + NGY) * P.pitch + NGX + i;
+    const double v = *p;
+    *p = v < P.z_min ? P.z_min : (v > P.z_max ? P.z_max : v);      // a NaN stays a NaN and is reported by the state checks
+}
+void launch_clamp_z1(const Params& P, double* q5, cudaStream_t s)
+{
+    dim3 grid((P.nx + 127) / 128, P.ny);
+    k_clamp_z1<<<grid, 128, 0, s>>>(P, q5);
+}
+
 // slab decomposition (sim_init_slab): cavity centres from global to slab-local columns
 __global__ void k_shift_cavities(Cav* __restrict__ cav, int n, double shift)
 {
@@ -70,7 +86,8 @@ __global__ void k_fill_state(const __grid_constant__ Params P, double* __restric
         W[0] = hug.rho1_s; W[1] = hug.rho_s; W[2] = hug.u_p; W[3] = 0.0; W[4] = p_shock; W[5] = P.z_min; W[6] = 0.0;
     } else {
         const double prof = q[5 * P.fstride + id];
-        W[0] = rho1_0; W[1] = rho2_0; W[2] = 0.0; W[3] = 0.0; W[4] = p0; W[5] = P.z_min + (1.0 - 2.0 * P.z_min) * prof; W[6] = 1.0;
+        W[0] = rho1_0; W[1] = rho2_0; W[2] = 0.0; W[3] = 0.0; W[4] = p0; W[6] = 1.0;
+        W[5] = fmin(fmax(P.z_min + (1.0 - 2.0 * P.z_min) * prof, P.z_min), P.z_max);
     }
     Face f;
     face_state(P, W, f);
