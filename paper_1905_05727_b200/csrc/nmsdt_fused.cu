@@ -6,14 +6,16 @@
 //                                                                     (k_xsweep<TRAIL> or k_ysweep<TRAIL>)
 // followed by the one-thread k_ctl (t += dt, next CFL dt).  Algorithmic HBM traffic: 2 x (7 read + 7 written) planes
 // = 224 B per cell-step.  The arithmetic is that of nmsdt_device.cuh (O3-O5) with the branch-free elementary
-// functions of nmsdt_math.cuh.
+// functions of nmsdt_math.cuh; a warp whose segment holds a cell that needs one of the rare rules (RK4 sub-steps R13,
+// first-order fallback R17, a density outside the power tables) repeats the segment with the exact rules.
 //
-//   k_ysweep: a thread owns a column and marches along y; the 3-cell primitive window, the previous right-face state
-//             and the half-finished update of the previous cell stay in registers; every load/store is a coalesced
-//             256-byte row piece and nothing is recomputed (4 ramp-up rows per segment).
+//   k_ysweep: a thread owns a column and marches along y; the primitive window and the previous right-face state live in
+//             thread-private shared-memory slots (value pairs, 128-bit accesses), the half-finished update of the previous
+//             cell in registers; every load/store is a coalesced 256-byte row piece and nothing is recomputed (4 ramp-up
+//             rows per segment).
 //   k_xsweep: a warp owns a row segment and marches along x in chunks of 64 cells, 2 adjacent cells per lane
 //             (128-bit loads/stores).  Neighbour primitives, the right-face state and the face flux cross lanes through
-//             three 33-slot rings in shared memory (slot = lane counter mod 33, so lane 31's entry of the previous
+//             three 33-slot rings of value pairs in shared memory (slot = lane counter mod 33, so lane 31's entry of the previous
 //             chunk is lane 0's left neighbour: no halo recomputation, no copies); 3 __syncwarp per chunk.
 #include "nmsdt_host.h"
 #include "nmsdt_fast.cuh"
@@ -234,8 +236,9 @@ constexpr int YT = 128;      // threads (columns) per block in k_ysweep
 constexpr int YST = 3;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1 in flight
 constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part (the math tables are static)
 
-// Per-thread state that lives across rows is kept in thread-private shared-memory slots ([..][YT] layout, conflict
-// free, no barriers): the staged input rows, the primitive window (cells c-2, c-1) and the previous right-face state.
+// Per-thread state that lives across rows is kept in thread-private shared-memory slots ([..][YT] layout of value pairs,
+// no barriers): the staged input rows, the primitive window (cell c-1 and its backward differences) and the previous
+// right-face state.
 // Only the half-finished update of cell c-1 stays in registers; this keeps the kernel at 128 registers (16 warps/SM).
 // One column segment of the y-sweep (rows c0 .. c0+seg-1 of column col); returns whether a cell asked for RK4
 // sub-stepping or the first-order fallback (EXACT = false only; the caller then redoes the segment with EXACT = true --
