@@ -253,17 +253,28 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     l0 = sim.launch_count()
-    sim.profile(True)
+    # Per-kernel device times for the roofline block come from an event pair around every kernel (sim_profile), which
+    # bypasses the CUDA-graph replay.  On the configs that do not fit L2 (C4, C5: milliseconds of kernels per step) that
+    # changes nothing and the pairs are recorded inside the timed region; the small, launch-bound configs (C1-C3) are
+    # timed the way a user runs them (graph replay) and their kernel shares are taken in a second, untimed pass.
+    profile_in_timed = 7 * cells * 8 > 126e6
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if profile_in_timed:
+        sim.profile(True)
     e0.record(sim.stream)
     sim.step(K)
     e1.record(sim.stream)
     barrier()
-    sim.profile(False)
+    if profile_in_timed:
+        sim.profile(False)
     launches = sim.launch_count() - l0
     ms = e0.elapsed_time(e1)
     sampler.stop_flag = True
     sampler.join(timeout=2)
+    if not profile_in_timed:
+        sim.profile(True)
+        sim.step(K)
+        sim.profile(False)
     kt = sim.kernel_times()
     d = sim.diagnostics()
     ms = max_over_ranks(ms, world, "cuda")
@@ -370,7 +381,8 @@ def main():
         "config": {"workload": "%s %dx%d, %d cavities, p_shock %.3g Pa, fp64 SoA 7 planes double-buffered; replicas only; "
                                "state %.1f MB > L2 (no flush needed)" % (args.config, g["nx"], g["ny"], ncav, cfg["init"]["p_shock"],
                                                                           7 * cells * 8 / 1e6),
-                   "variant": args.variant, "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
+                   "variant": args.variant, "kernel_timing": "event pairs inside the timed region" if profile_in_timed else
+                   "timed region = CUDA-graph replay; kernel event pairs in a second pass", "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "burned_mass": d["burned_mass"]},
         "post": post, "slab": slab_block,
