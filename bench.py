@@ -379,9 +379,9 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s %dx%d, %d cavities, p_shock %.3g Pa, fp64 SoA 7 planes double-buffered; replicas only; "
-                               "state %.1f MB > L2 (no flush needed)" % (args.config, g["nx"], g["ny"], ncav, cfg["init"]["p_shock"],
-                                                                          7 * cells * 8 / 1e6),
-                   "variant": args.variant, "kernel_timing": "event pairs inside the timed region" if profile_in_timed else
+                               "state %.1f MB %s" % (args.config, g["nx"], g["ny"], ncav, cfg["init"]["p_shock"], 7 * cells * 8 / 1e6,
+                                                     "> L2 (no flush needed)" if 7 * cells * 8 > 126e6 else "fits the 126 MB L2 (small config, not a bench line)"),
+                   "variant": args.variant, "ranks_share_a_gpu": bool(shared_gpu), "kernel_timing": "event pairs inside the timed region" if profile_in_timed else
                    "timed region = CUDA-graph replay; kernel event pairs in a second pass", "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "burned_mass": d["burned_mass"]},
