@@ -209,6 +209,7 @@ __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double la
 #endif
 constexpr int XW = 4;                       // warps per block in k_xsweep
 constexpr int RING = 33;
+constexpr int XRAMP = 4;                    // cells left of a segment that k_xsweep recomputes (stencil radius 2, two passes of neighbours)
 constexpr int RING_DOUBLES = (16 + 10 + 8) * RING;
 constexpr int PRING = 66;                   // staged input pairs: chunk k (32 slots), chunk k+1 in flight, lane 31 of chunk k-1
 constexpr int XS_DOUBLES = XW * (RING_DOUBLES + 7 * PRING * 2);    // dynamic part (the math tables are static)
@@ -411,25 +412,26 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
     const double* rin = qin + (long long)(row + NGY) * P.pitch + NGX;
     double* rout = qout + (long long)(row + NGY) * P.pitch + NGX;
     const int nxe = (P.nx + 1) & ~1;                 // last pair base that is ever needed (cell nx+1 is the outer ghost; for odd nx the pair ends in row padding)
-    const int niter = (c1 - c0 + 63) >> 6;
+    const int niter = (c1 - c0 + XRAMP + 63) >> 6;   // chunks of 64 cells, the first one starts XRAMP = 4 cells left of c0
     const bool fixed_in = (MODE == MODE_LEAD) && (P.bc_xlo == 3);
     int sw = lane;                                   // ring slot written by this lane: (32 k + lane) mod 33
     int ps = lane;                                   // staging slot of this lane's pair: (32 k + lane) mod 66
-    {   // stage chunk 0 (cells c0-62 .. c0+1; only lanes 30, 31 are used)
-        const int Ac = min(max(c0 - 64 + 2 * lane + 2, -2), nxe);
+    {   // stage chunk 0 (cells c0-2 .. c0+61)
+        const int Ac = min(max(c0 - XRAMP + 2 * lane + 2, -2), nxe);
 #pragma unroll
         for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + ps), rin + Ac + f * fs);
         cp_async_commit();
     }
-    for (int k = 0; k <= niter; ++k) {
-        const int b = c0 + 64 * (k - 1);             // first cell updated in this iteration
+    for (int k = 0; k < niter; ++k) {
+        const int b = c0 - XRAMP + 64 * k;           // first cell this iteration would update
         const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
-        // iteration 0 only primes the rings (cells c0-2 .. c0+1 through lanes 30, 31); the body is branch free and
-        // simply runs on clamped / not-yet-valid data there, nothing of which is stored
+        // In iteration 0 lanes 0, 1 hold the left stencil cells c0-2 .. c0+1: they have no (complete) left neighbours of
+        // their own, so what they would update (cells c0-4 .. c0-1, another segment's) is not stored; the body is branch
+        // free and simply runs on not-yet-valid ring data there.  Like the y-sweep, a segment costs 4 ramp-up cells.
         const int sr = sw == 0 ? RING - 1 : sw - 1;  // left neighbour's slot
         FCell WA, WB;
         const int psn = ps + 32 >= PRING ? ps + 32 - PRING : ps + 32;
-        if (k < niter) {                             // stage the next chunk while this one is computed
+        if (k + 1 < niter) {                         // stage the next chunk while this one is computed
             const int An = min(A + 64, nxe);
 #pragma unroll
             for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + psn), rin + An + f * fs);
@@ -501,7 +503,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
         const int u0 = b + 2 * lane;
         {
-            const bool valid = k > 0 && u0 < c1;
+            const bool valid = u0 >= c0 && u0 < c1;
             double F0[8];
 #pragma unroll
             for (int f = 0; f < 4; ++f) { const double2 v = rf[f * RING + sr]; F0[2 * f] = v.x; F0[2 * f + 1] = v.y; }
@@ -640,6 +642,24 @@ static int pick_seg(int n, int unit, int target, int ramp, int lines, int slots)
     return best_seg;
 }
 
+// x-sweep: a segment of 64 m - XRAMP cells takes exactly m marching iterations of 64 cells (the first chunk starts XRAMP
+// cells to the left); pick the m that minimises waves x (iterations + 2): a block's start (table copy, first staged chunk)
+// costs about two iterations.  Segment starts stay even (128-bit pair loads).
+static int pick_seg_x(int n, int lines, int slots)
+{
+    const int mmax = (n + XRAMP + 63) / 64;                    // one segment for the whole row
+    int best = 64 * mmax - XRAMP; double bestc = 1e300;
+    for (int m = 2; m <= mmax; ++m) {
+        const int seg = 64 * m - XRAMP;
+        if (seg > 4096 && m < mmax) continue;                  // segments of at most a few thousand cells, or the whole row
+        const int nseg = (n + seg - 1) / seg;
+        const double waves = (double)(((long long)lines * nseg + slots - 1) / slots);
+        const double cost = waves * (m + 2.0);
+        if (cost < bestc * (1.0 - 1e-9)) { bestc = cost; best = seg; }
+    }
+    return best;
+}
+
 static int num_sms()
 {
     static int n = 0;
@@ -701,7 +721,7 @@ void launch_sweep_fused(const Params& P, const double* qin, double* qout, const 
     const int lim = P.limiter == 0 ? 0 : 1;
     if (dir == 0) {
         const int lines = (P.ny + XW - 1) / XW;
-        const int seg = pick_seg(P.nx, 64, 2048, 64, lines, num_sms() * NMSDT_X_MINBLOCKS);
+        const int seg = pick_seg_x(P.nx, lines, num_sms() * NMSDT_X_MINBLOCKS);
         sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, P, qin, qout, dtp, ctl, seg);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
