@@ -530,15 +530,13 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
                 bad |= (valid ? bad1 : 0) | ((valid && two) ? bad2 : 0);
                 hot |= (valid && hot1) || (valid && two && hot2);
             }
+            // always a 128-bit pair store: only the last pair of a row with odd nx has a second cell that is not a cell, and that
+            // one is the ghost column nx of the output planes, which the halo step (or the slab exchange) rewrites before any
+            // x-sweep reads it and which nothing else reads
             double* po = rout + u0;
             if (valid) {
-                if (two) {
 #pragma unroll
-                    for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
-                } else {
-#pragma unroll
-                    for (int f = 0; f < 7; ++f) po[f * fs] = oa[f];
-                }
+                for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
             }
         }
         sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
