@@ -34,14 +34,14 @@ from paper_1905_05727_b200 import inputs  # noqa: E402
 METRIC = "fp64 cell-updates/s per 2D step"
 UNIT = "cell-updates/s"
 # algorithmic FP64 work of one cell in one fused directional sweep, from ncu's counters of the
-# C5 launches (profiles/r01i_fused_c5.md) divided by the ramp-up redundancy of a segment (65/64 on C5).
+# C5 launches (profiles/r01j_fused_c5.md) divided by the ramp-up redundancy of a segment (65/64 on C5).
 #   FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot):
 FP64_INSTR_PER_CELL = {"lead": 351.0, "trail": 413.0}       # pass 1 = S + sweep; pass 2 = sweep + S + wavespeed
 #   flops with dadd = dmul = 1, dfma = 2, dsetp = 0 (54 % of the FP64 instructions are DFMA):
 FLOP_PER_CELL = {"lead": 524.0, "trail": 617.0}
 FP64_LANES_PER_SM, N_SM = 64, 148
 # dram__bytes_read.sum + dram__bytes_write.sum per cell per launch from the ncu --set full capture of C5 (mean of the
-# lead and trail launches; profiles/r01i_fused_c5.md): 113.0 B (x), 112.6 B (y) against 112 B algorithmic
+# lead and trail launches; profiles/r01j_fused_c5.md): 113.0 B (x), 112.6 B (y) against 112 B algorithmic
 TRAFFIC_BYTES_PER_CELL = {"sweep_x": 112.95, "sweep_y": 112.6}
 
 
