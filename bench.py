@@ -307,6 +307,10 @@ def main():
             "peak_source": "148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (guide's unit counts and clock)",
             "peak_measured_dfma_probe": probe_gflops / 1e3 if probe_gflops else None,
             "whole_step_frac": 2.0 * step_instr * cells * K / (ms * 1e-3) / 1e12 / peak_tflops,
+            # the same against the peak at the SM clock nvidia-smi reported during the timed region (the step runs close to the
+            # board's power limit: sw_power_cap lowers the clock by a few per cent on some boards)
+            "whole_step_frac_at_measured_clock": (2.0 * step_instr * cells * K / (ms * 1e-3) / 1e12 / peak_tflops * sm_max / clk["sm_mhz"]
+                                                  if clk.get("sm_mhz") else None),
             "ms_per_launch": dom_ms,
             "hbm_gbs_algorithmic": 112.0 * cells / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0,
             "hbm_peak_gbs": pk.get("hbm_gbs", 6650.0),
