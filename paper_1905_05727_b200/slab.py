@@ -58,8 +58,6 @@ def slab_grid(grid, rank, world):
         g["bc_xlo"] = BC_EXTERNAL
     if hi is not None:
         g["bc_xhi"] = BC_EXTERNAL
-    if world > 1 and grid["bc_xlo"] == BC_PERIODIC and lo is None:      # not reachable: periodic x wraps
-        raise AssertionError
     return g, x0
 
 
