@@ -326,6 +326,38 @@ def test_rare_paths_first_order_fallback(O, B, d, variant):
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("ratio", [0.7, 1.6])
+def test_non_square_cells(O, B, ratio, variant):
+    """dy = ratio * dx: the y-sweep's dt/dy, the CFL step's min(dx, dy) (R11) and the diagnostics' dx dy, on a developed
+    cavity collapse (the oracle side is pinned on such grids by tests/test_oracle_cfl.py)"""
+    cfg, o0 = _developed_c1(O, reactive=1, steps=400)
+    g = dict(cfg["grid"], dy=ratio * cfg["grid"]["dx"])
+    o = O.Oracle(g, cfg["eos"], cfg["kin"], threads=8)
+    o.init_fields(o0.state())
+    s = B.Sim(g, cfg["eos"], cfg["kin"], variant=variant)
+    _sync_state(o, s)
+    dt = o.cfl_dt()
+    assert s.cfl_dt() == pytest.approx(dt, rel=1e-13)
+    assert dt == pytest.approx(0.4 * min(g["dx"], g["dy"]) / o.diagnostics()["smax"], rel=1e-13)
+    for d in (0, 1):
+        o.sweep(d, dt), s.sweep(d, dt)
+        _assert_one_step(o, s, what="sweep %d, dy = %g dx" % (d, ratio))
+        o.init_fields(o0.state())
+        _sync_state(o, s)
+    for it in range(2):
+        o.step(1), s.step(1)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="step %d, dy = %g dx" % (it, ratio))
+    da, db = s.diagnostics(), o.diagnostics()
+    for k in ("t", "dt_last", "M2r", "mass1", "mass2", "momx", "energy", "rate_inst", "smax"):
+        assert da[k] == pytest.approx(db[k], rel=1e-12), k
+    # the cell shape matters: the same two steps on square cells give another state
+    o_sq = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"], threads=8)
+    o_sq.init_fields(o0.state())
+    o_sq.step(2)
+    assert max(rel_diff(o_sq.state(), o.state(), o.read_field("c"))) > 1e-4
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_500_steps_l1_parity_c1(O, B, variant):
     cfg = inputs.config("C1", reactive=1)
     o, s = _pair(O, B, cfg, variant=variant)
