@@ -133,6 +133,17 @@ int sim_diagnostics(sim_t*, sim_diag_t* out);
 int sim_read_field(sim_t*, int field_id, double* host_out);
 /* Cavity list used by the last sim_init (generator parity). Writes min(n, cap) entries. [sync] */
 int sim_get_cavities(sim_t*, sim_cavity_t* host_out, int cap, int* n);
+/* Seeded generator (R16; Eq. 8) of the last sim_init: the air fraction asked for and the one placed,
+   pi sum r_k^2 / ((x_hi - x_lo) ny); both 0 when the layout was a list or a lattice.  sim_init returns SIM_ERR_ARG (and
+   leaves the handle uninitialised) when the generator spends its candidate budget, 256 candidates per cavity of the
+   target, before reaching the target: the list would silently describe another porosity.  These two numbers then say
+   by how much. */
+int sim_cavity_stats(const sim_t*, double* phi_target, double* phi_achieved);
+/* Fused variant: how many warp segments the sweep kernels have repeated with the exact rules since the last sim_init*
+   (a cell asked for RK4 sub-steps R13, for the first-order fallback R17, or held a liquid density outside the tables of
+   the x^C, x^D evaluation).  0 on every run of the BASELINE configs; a large count means the fast
+   path is being paid twice. [sync] */
+int sim_redo_count(sim_t*, long long* n);
 
 /* ---- post-processing of the state (the paper's analysis figures; R23-R26).  Not part of sim_step. ----
  * sim_profiles: y-averaged profiles Eq. 9-11 by the midpoint rule over the ny rows,

@@ -313,7 +313,10 @@ extern "C" int orc_gen_cavities(unsigned long long seed, double phi, double dmin
     const int64_t H = (int64_t)ny * 256;
     const int64_t target = (int64_t)std::floor(phi * (double)(x_hi - x_lo) * (double)ny * 65536.0 / 3.14159265358979323846);
     if (Rmin <= 0 || Rmax < Rmin || x_hi <= x_lo || ny <= 0) return -1;
-    const int64_t max_cand = 16 * (target / (Rmin * Rmin) + 1) + 1024;
+    /* candidate budget: 256 candidates per cavity of the target.  The paper's densest case (phi = 8 %, centre spacing
+       2.5 d_c) fills 0.50 of the plane with exclusion disks, close to the ~0.547 jamming limit of random
+       sequential placement, and needs ~40 candidates per cavity; a target beyond the jamming limit ends here. */
+    const int64_t max_cand = 256 * (target / (Rmin * Rmin) + 1) + 1024;
     std::vector<int64_t> X, Y, R;
     int64_t sum = 0;
     for (int64_t k = 0; k < max_cand && sum < target; ++k) {

@@ -21,7 +21,7 @@ FIELD = {"q0": 0, "q1": 1, "q2": 2, "q3": 3, "q4": 4, "q5": 5, "q6": 6, "p": 16,
 # every symbol include/nmsdt.h declares (tests check that the library exports each one)
 SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error", "sim_init", "sim_init_fields",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
-           "sim_read_field", "sim_get_cavities", "sim_set_variant", "sim_launch_count", "sim_device_layout",
+           "sim_read_field", "sim_get_cavities", "sim_cavity_stats", "sim_redo_count", "sim_set_variant", "sim_launch_count", "sim_device_layout",
            "sim_probe_fp64", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
            "sim_shock_kinematics", "sim_init_slab", "sim_slab_halo_bytes", "sim_slab_begin", "sim_slab_smax_ptr",
            "sim_slab_ctl", "sim_slab_pass_dir", "sim_slab_pass", "sim_slab_pack", "sim_slab_unpack", "sim_slab_info",
@@ -105,6 +105,8 @@ def load_library():
         "sim_diagnostics": (C.c_int, [vp, C.POINTER(Diag)]),
         "sim_read_field": (C.c_int, [vp, C.c_int, dp]),
         "sim_get_cavities": (C.c_int, [vp, C.POINTER(Cavity), C.c_int, C.POINTER(C.c_int)]),
+        "sim_cavity_stats": (C.c_int, [vp, dp, dp]),
+        "sim_redo_count": (C.c_int, [vp, C.POINTER(C.c_longlong)]),
         "sim_set_variant": (C.c_int, [vp, C.c_int, C.c_int]),
         "sim_launch_count": (C.c_longlong, [vp]),
         "sim_device_layout": (C.c_int, [vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(C.c_int),
@@ -265,6 +267,17 @@ class Sim:
         arr = (Cavity * max(n.value, 1))()
         self._chk(self.L.sim_get_cavities(self.h, arr, n.value, C.byref(n)), "sim_get_cavities")
         return np.array([[arr[i].x, arr[i].y, arr[i].r] for i in range(n.value)], dtype=np.float64).reshape(-1, 3)
+
+    def cavity_stats(self):
+        """(air fraction asked of the seeded generator, air fraction placed); (0, 0) for a list or a lattice"""
+        a, b = C.c_double(), C.c_double()
+        self._chk(self.L.sim_cavity_stats(self.h, C.byref(a), C.byref(b)), "sim_cavity_stats")
+        return a.value, b.value
+
+    def redo_count(self):
+        n = C.c_longlong()
+        self._chk(self.L.sim_redo_count(self.h, C.byref(n)), "sim_redo_count")
+        return n.value
 
     def set_variant(self, variant, use_graph=True):
         self._chk(self.L.sim_set_variant(self.h, int(variant), int(bool(use_graph))), "sim_set_variant")

@@ -20,7 +20,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct Layout {
     int pitch, rows;
     long long fstride;       // doubles
-    size_t off_A, off_B, off_inflow, off_partial, off_diag, off_ctl, off_scratch, off_tab, total;
+    size_t off_A, off_B, off_inflow, off_partial, off_diag, off_diag0, off_ctl, off_scratch, off_tab, total;
 };
 
 Layout make_layout(int nx, int ny)
@@ -36,6 +36,7 @@ Layout make_layout(int nx, int ny)
     L.off_inflow = o; o = align_up(o + (size_t)7 * ny * sizeof(double), 256);
     L.off_partial = o; o = align_up(o + (size_t)DIAG_BLOCKS * (DIAG_NV + 1) * sizeof(double), 256);
     L.off_diag = o; o = align_up(o + sizeof(DiagOut), 256);
+    L.off_diag0 = o; o = align_up(o + sizeof(DiagOut), 256);
     L.off_ctl = o; o = align_up(o + sizeof(Ctl), 256);
     L.off_scratch = o; o = align_up(o + 8 * sizeof(double), 256);
     L.off_tab = o; o = align_up(o + MATH_TAB_DOUBLES_LOG * sizeof(double), 256);
@@ -64,6 +65,9 @@ struct sim {
     bool inited = false;
     long long host_step = 0;        // mirrors ctl->step (step parity decides the sweep order)
     double M2tot0 = 0.0;
+    bool m2tot0_pending = false;    // the reduction of the initial state is queued in d_diag0 and not read back yet
+    DiagOut* d_diag0 = nullptr;
+    double phi_target = 0.0, phi_achieved = 0.0;    // seeded generator: air fraction asked for / placed (0 without a generator)
     int variant = SIM_VARIANT_FUSED;
     int use_graph = 1;
     cudaGraphExec_t gexec = nullptr;    // fused path: one even (X-Y) + one odd (Y-X) step = 10 kernel nodes
@@ -132,31 +136,60 @@ void fill_params(sim* s)
     P.Ta = k.Ta; P.Cpre = k.Cpre; P.Q = k.Q; P.theta0 = k.substep_theta; P.reactive = k.reactive; P.max_substeps = k.max_substeps;
 }
 
-// host-side scalar model functions for the Hugoniot root find (O7)
-double h_pref(const sim_eos_t& e, double rho) { double x = rho / e.rho02; return e.A * std::pow(x, e.C) - e.B * std::pow(x, e.D); }
-double h_eref(const sim_eos_t& e, double rho)
-{
-    double x = rho / e.rho02;
-    return -e.A / (e.rho02 * (1.0 - e.C)) * (std::pow(x, e.C - 1.0) - 1.0) + e.B / (e.rho02 * (1.0 - e.D)) * (std::pow(x, e.D - 1.0) - 1.0);
-}
-double h_e2(const sim_eos_t& e, double rho, double p) { return h_eref(e, rho) + (p - h_pref(e, rho)) / (rho * e.Gamma2); }
+// Shocked-slab state (O7): the neat-liquid Hugoniot point at pressure ps, found in the specific volume v = 1/rho.
+// With Eq. 2 solved for e (constant Gamma2) the Hugoniot condition e - e0 = (ps + p0)(v0 - v)/2 reads
+//     h(v) = e_ref(v) + v (ps - p_ref(v))/Gamma2 - e0 - (ps + p0)(v0 - v)/2 = 0,
+// and since Eq. 3-4 satisfy de_ref/dv = -p_ref,
+//     h'(v) = -p_ref + (ps - p_ref)/Gamma2 - v p_ref'(v)/Gamma2 + (ps + p0)/2,   v p_ref'(v) = -(A C x^C - B D x^D),  x = 1/(rho02 v).
+// Newton from v0, kept inside a bracket that every iterate tightens (h(v0) > 0 for ps > p0; h < 0 towards the compression
+// limit v0 Gamma2/(Gamma2 + 2)); written apart from the oracle's bisection in rho.
+struct HugFn {
+    const sim_eos_t& e; double ps, p0, v0, e0;
+    static void ref(const sim_eos_t& e, double v, double& pr, double& er, double& vdpr)
+    {
+        const double x = 1.0 / (e.rho02 * v), xC = std::pow(x, e.C), xD = std::pow(x, e.D);
+        pr = e.A * xC - e.B * xD;                                                              // Eq. 3
+        er = (-e.A / (1.0 - e.C) * (xC / x - 1.0) + e.B / (1.0 - e.D) * (xD / x - 1.0)) / e.rho02;   // Eq. 4
+        vdpr = -(e.A * e.C * xC - e.B * e.D * xD);
+    }
+    void eval(double v, double& h, double& dh) const
+    {
+        double pr, er, vdpr;
+        ref(e, v, pr, er, vdpr);
+        h = er + v * (ps - pr) / e.Gamma2 - e0 - 0.5 * (ps + p0) * (v0 - v);
+        dh = -pr + (ps - pr) / e.Gamma2 - vdpr / e.Gamma2 + 0.5 * (ps + p0);
+    }
+};
 
 bool hugoniot(const sim_eos_t& e, double p0, double rho1_0, double rho2_0, double ps, Hug& out)
 {
-    const double e0 = h_e2(e, rho2_0, p0), v0 = 1.0 / rho2_0;
-    auto f = [&](double rho) { return h_e2(e, rho, ps) - e0 - 0.5 * (ps + p0) * (v0 - 1.0 / rho); };
-    double lo = rho2_0 * (1.0 + 1e-12), hi = rho2_0 * 1.5;
-    if (!(ps > p0) || !(f(lo) > 0.0)) return false;
-    int guard = 0;
-    while (f(hi) > 0.0) { hi *= 1.5; if (++guard > 40) return false; }
-    for (int it = 0; it < 200; ++it) { double mid = 0.5 * (lo + hi); if (f(mid) > 0.0) lo = mid; else hi = mid; }
-    const double rs = 0.5 * (lo + hi);
+    if (!(ps > p0) || !(rho2_0 > 0.0)) return false;
+    const double v0 = 1.0 / rho2_0;
+    double pr0, er0, t0;
+    HugFn::ref(e, v0, pr0, er0, t0);
+    const HugFn F{e, ps, p0, v0, er0 + v0 * (p0 - pr0) / e.Gamma2};
+    double hi = v0, lo = v0 * e.Gamma2 / (e.Gamma2 + 2.0) * 0.5, h, dh;
+    F.eval(lo, h, dh);
+    for (int it = 0; it < 60 && !(h < 0.0); ++it) { lo *= 0.5; F.eval(lo, h, dh); }
+    if (!(h < 0.0)) return false;
+    double v = 0.5 * (lo + hi);
+    for (int it = 0; it < 200; ++it) {
+        F.eval(v, h, dh);
+        if (h > 0.0) hi = v; else lo = v;
+        double vn = v - h / dh;
+        if (!(vn > lo && vn < hi)) vn = 0.5 * (lo + hi);            // safeguard: bisect when Newton leaves the bracket
+        if (std::fabs(vn - v) <= 1e-16 * v) { v = vn; break; }
+        v = vn;
+    }
+    const double rs = 1.0 / v;
+    double prs, ers, ts;
+    HugFn::ref(e, v, prs, ers, ts);
     out.rho_s = rs;
-    out.u_p = std::sqrt((ps - p0) * (v0 - 1.0 / rs));
-    out.U_s = out.u_p / (1.0 - rho2_0 / rs);
-    out.T2_s = e.Tref2 + (ps - h_pref(e, rs)) / (rs * e.Gamma2 * e.cv2);
+    out.u_p = std::sqrt((ps - p0) * (v0 - v));
+    out.U_s = v0 * std::sqrt((ps - p0) / (v0 - v));                 // mass + momentum jump: (rho0 U_s)^2 = (ps - p0)/(v0 - v)
+    out.T2_s = e.Tref2 + (ps - prs) * v / (e.Gamma2 * e.cv2);       // Eq. 5
     const double g = e.gamma1;
-    out.rho1_s = rho1_0 * ((g + 1.0) * ps + (g - 1.0) * p0) / ((g - 1.0) * ps + (g + 1.0) * p0);
+    out.rho1_s = rho1_0 * ((g + 1.0) * ps + (g - 1.0) * p0) / ((g - 1.0) * ps + (g + 1.0) * p0);    // trace air: its own shock Hugoniot
     return true;
 }
 
@@ -249,22 +282,22 @@ void prepare_ctl_fused(sim* s)
     s->launches += 2;
 }
 
+// End of sim_init / sim_init_fields: inflow column, control block and the reduction of the initial state (M2tot0 of
+// Eq. 13 is M2r at t = 0) are queued behind the caller's data; the one synchronisation that follows also ends the
+// library's use of the caller's host buffers.  The reduced sums stay on the device until the first sim_diagnostics.
 int finish_init(sim* s)
 {
     cudaStream_t st = s->stream;
     launch_capture_inflow(s->P, s->A, s->inflow, st);
-    Ctl h; std::memset(&h, 0, sizeof(h));
-    cudaMemcpyAsync(s->ctl, &h, sizeof(Ctl), cudaMemcpyHostToDevice, st);
-    cudaStreamSynchronize(st);
+    cudaMemsetAsync(s->ctl, 0, sizeof(Ctl), st);
+    launch_diag(s->P, s->A, s->partial, s->d_diag0, st);
+    s->launches += 3;
     s->host_step = 0;
-    s->inited = true;
     s->cfl_valid = false;
-    s->launches += 1;
-    sim_diag_t d;
     s->M2tot0 = 0.0;
-    int rc = sim_diagnostics(s, &d);
-    if (rc != SIM_OK && rc != SIM_ERR_BAD) return rc;
-    s->M2tot0 = d.M2r;
+    s->m2tot0_pending = true;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return check_cuda(s, "init");
+    s->inited = true;
     return check_cuda(s, "init");
 }
 
@@ -306,7 +339,7 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     }
     s->A = (double*)(s->base + s->L.off_A); s->B = (double*)(s->base + s->L.off_B);
     s->inflow = (double*)(s->base + s->L.off_inflow); s->partial = (double*)(s->base + s->L.off_partial);
-    s->d_diag = (DiagOut*)(s->base + s->L.off_diag); s->ctl = (Ctl*)(s->base + s->L.off_ctl);
+    s->d_diag = (DiagOut*)(s->base + s->L.off_diag); s->d_diag0 = (DiagOut*)(s->base + s->L.off_diag0); s->ctl = (Ctl*)(s->base + s->L.off_ctl);
     s->scratch = (double*)(s->base + s->L.off_scratch);
     s->tab = (double*)(s->base + s->L.off_tab);
     fill_params(s);
@@ -342,8 +375,9 @@ static int init_common(sim_t* s, const sim_init_t* in, int x0, bool slab)
     if (in->shock_cells < 0 || (!slab && in->shock_cells > s->g.nx) || !(in->interface_width > 0.0)) return fail(s, SIM_ERR_ARG, "sim_init: bad shock_cells / interface_width");
     cudaStream_t st = s->stream;
     const Params& P = s->P;
+    s->inited = false;              // until finish_init: a failed sim_init leaves no half-written state behind a valid handle
     if (s->d_cav) { cudaFree(s->d_cav); s->d_cav = nullptr; }
-    s->ncav = 0;
+    s->ncav = 0; s->phi_target = s->phi_achieved = 0.0;
     std::vector<Cav> host;
     if (in->cav && in->ncav > 0) {
         for (int i = 0; i < in->ncav; ++i) host.push_back({in->cav[i].x - x0, in->cav[i].y, in->cav[i].r});
@@ -353,11 +387,21 @@ static int init_common(sim_t* s, const sim_init_t* in, int x0, bool slab)
         for (int jj = 0; sp * (jj + 1) <= (double)s->g.ny; ++jj)
             for (int ii = 0; in->x_lo + sp * (ii + 1) <= (double)in->x_hi; ++ii) host.push_back({in->x_lo + 0.5 * sp + sp * ii - x0, 0.5 * sp + sp * jj, r});
     } else if (in->phi > 0.0) {
+        long long sum_r2 = 0, target_r2 = 0;
         int n = generate_cavities(in->seed, in->phi, in->dmin, in->dmax, in->min_gap, in->x_lo, in->x_hi, s->g.ny,
-                                  s->g.bc_ylo == SIM_BC_PERIODIC ? 1 : 0, &s->d_cav, st, &s->launches);
+                                  s->g.bc_ylo == SIM_BC_PERIODIC ? 1 : 0, &s->d_cav, st, &s->launches, &sum_r2, &target_r2);
         if (n == -1) return fail(s, SIM_ERR_ARG, "sim_init: bad generator parameters");
         if (n < 0) { cudaGetLastError(); return fail(s, SIM_ERR_CUDA, "sim_init: cavity generator failed"); }
         s->ncav = n;
+        // air fraction placed: pi sum r^2 over the seeded region (r in 1/256 cell)
+        const double region = (double)(in->x_hi - in->x_lo) * (double)s->g.ny * 65536.0 / 3.14159265358979323846;
+        s->phi_target = in->phi; s->phi_achieved = (double)sum_r2 / region;
+        if (sum_r2 < target_r2) {
+            char msg[256];
+            std::snprintf(msg, sizeof msg, "sim_init: the seeded generator placed %d cavities = air fraction %.5f of the %.5f asked for "
+                          "(candidate budget spent: the target is at or beyond the jamming limit of this minimum gap)", n, s->phi_achieved, in->phi);
+            return fail(s, SIM_ERR_ARG, msg);
+        }
         if (x0 != 0 && n > 0) { launch_shift_cavities(s->d_cav, n, -(double)x0, st); s->launches++; }
     }
     if (!host.empty()) {
@@ -391,10 +435,10 @@ int sim_init_fields(sim_t* s, const double* const host_q[7])
     }
     launch_clamp_z1(P, s->A + 5 * P.fstride, s->stream);       // q5 within [z_min, 1 - z_min]: the invariant of every stored state
     s->launches++;
-    cudaStreamSynchronize(s->stream);
+    const int rc = finish_init(s);                              // (synchronises: the host planes are free again)
     if (s->d_cav) { cudaFree(s->d_cav); s->d_cav = nullptr; }
-    s->ncav = 0;
-    return finish_init(s);
+    s->ncav = 0; s->phi_target = s->phi_achieved = 0.0;
+    return rc;
 }
 
 int sim_cfl_dt(sim_t* s, double* dt_out)
@@ -496,11 +540,13 @@ int sim_diagnostics(sim_t* s, sim_diag_t* out)
     if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_diagnostics: not initialised");
     launch_diag(s->P, s->A, s->partial, s->d_diag, s->stream);
     s->launches += 2;
-    DiagOut d; Ctl c;
+    DiagOut d, d0; Ctl c;
+    if (s->m2tot0_pending) cudaMemcpyAsync(&d0, s->d_diag0, sizeof(DiagOut), cudaMemcpyDeviceToHost, s->stream);
     cudaMemcpyAsync(&d, s->d_diag, sizeof(DiagOut), cudaMemcpyDeviceToHost, s->stream);
     cudaMemcpyAsync(&c, s->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s->stream);
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_diagnostics");
     const double dA = s->g.dx * s->g.dy;
+    if (s->m2tot0_pending) { s->M2tot0 = d0.sum[5] * dA; s->m2tot0_pending = false; }
     out->t = c.t; out->step = c.step; out->dt_last = c.dt_last; out->smax = d.smax;
     out->M2r = d.sum[5] * dA; out->M2tot0 = s->M2tot0; out->burned_mass = s->M2tot0 - out->M2r; out->rate_inst = d.sum[6] * dA;
     out->mass1 = d.sum[0] * dA; out->mass2 = d.sum[1] * dA; out->momx = d.sum[2] * dA; out->momy = d.sum[3] * dA; out->energy = d.sum[4] * dA;
@@ -537,6 +583,24 @@ int sim_get_cavities(sim_t* s, sim_cavity_t* host_out, int cap, int* n)
         cudaMemcpyAsync(host_out, s->d_cav, sizeof(Cav) * (size_t)m, cudaMemcpyDeviceToHost, s->stream);
         if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_get_cavities");
     }
+    return SIM_OK;
+}
+
+int sim_cavity_stats(const sim_t* s, double* phi_target, double* phi_achieved)
+{
+    if (!s) return SIM_ERR_ARG;
+    if (phi_target) *phi_target = s->phi_target;
+    if (phi_achieved) *phi_achieved = s->phi_achieved;
+    return SIM_OK;
+}
+
+int sim_redo_count(sim_t* s, long long* n)
+{
+    if (!s || !n) return fail(s, SIM_ERR_ARG, "sim_redo_count: NULL argument");
+    Ctl c;
+    cudaMemcpyAsync(&c, s->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_redo_count");
+    *n = c.redo;
     return SIM_OK;
 }
 

@@ -44,7 +44,7 @@ struct Ctl {
     long long step;
     unsigned long long smax_bits; // max wavespeed of the current state, as ordered bits of a non-negative double
     int bad;
-    int pad;
+    int redo;                     // fused path: warp segments repeated with the exact rules since sim_init (R13 / R17 / power tables)
 };
 
 __device__ __forceinline__ double clampd(double x, double lo, double hi) { return x < lo ? lo : (x > hi ? hi : x); }

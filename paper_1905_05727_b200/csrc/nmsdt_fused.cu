@@ -194,10 +194,12 @@ __device__ __forceinline__ void reduce_smax(double smax, int bad, Ctl* ctl)
 }
 
 // post-source conserved values of a cell whose post-source lambda is known (pass 1 applies S on load, O6)
+// O5 moves q1 Q (lam0 - lam1) with lam0 = clamp(q6/q1, 0, 1) (O3): q1 lam0 = q6 clamped to [0, q1]
 __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double lam1)
 {
     const double q6n = q[1] * lam1;
-    q[4] = fma(P.Q, q[6] - q6n, q[4]);
+    const double q6c = hi_word(q[6]) < 0 ? 0.0 : dmin_(q[6], q[1]);
+    q[4] = fma(P.Q, q6c - q6n, q[4]);
     q[6] = q6n;
 }
 
@@ -379,6 +381,7 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
     if (col < P.nx) {
         const bool redo = y_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_dyn, smax, bad);
         if (__any_sync(__activemask(), redo)) {                  // rare: redo the warp's segment with the exact R13 / R17 rules
+            if ((threadIdx.x & 31) == 0) atomicAdd(&ctl->redo, 1);
             smax = 0.0; bad = 0;
             y_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_dyn, smax, bad);
         }
@@ -470,15 +473,21 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             }
             lam_u0 = Wmm.lam; lam_u1 = Wm1.lam;
             double WL[7], WR[7];
-            bool oor = false;                        // a face density outside the power tables
-            recon_fast<LIM, EXACT>(P, Wmm, Wm1, WA, khalf, WL, WR, k > 0 || lane > 0, hot);   // (k = 0, lane 0: the left slot is not written yet)
-            face_fast<EXACT>(P, s_tab, WL, FL1, oor);
-            face_fast<EXACT>(P, s_tab, WR, FR1, oor);
-            recon_fast<LIM, EXACT>(P, Wm1, WA, WB, khalf, WL, WR, k > 0 || lane > 0, hot);
-            face_fast<EXACT>(P, s_tab, WL, FL2, oor);
+            // What may ask for a redo: reconstructions whose window is real (k = 0, lane 0: the left slot is not written yet)
+            // and whose cell is at most the ghost cell nx, the last one a stored face needs.  Cell nx + 1 is reconstructed
+            // from cell nx + 2, which does not exist: row padding when nx is odd (its NaN primitives would raise the
+            // out-of-table flag on every row end), a clamped reload otherwise.
+            const bool real = k > 0 || lane > 0;
+            const bool cnt1 = real && A - 1 <= P.nx, cnt2 = real && A <= P.nx;
+            bool oor1 = false, oor2 = false;         // a face density outside the power tables
+            recon_fast<LIM, EXACT>(P, Wmm, Wm1, WA, khalf, WL, WR, cnt1, hot);
+            face_fast<EXACT>(P, s_tab, WL, FL1, oor1);
+            face_fast<EXACT>(P, s_tab, WR, FR1, oor1);
+            recon_fast<LIM, EXACT>(P, Wm1, WA, WB, khalf, WL, WR, cnt2, hot);
+            face_fast<EXACT>(P, s_tab, WL, FL2, oor2);
             FFace FR2;
-            face_fast<EXACT>(P, s_tab, WR, FR2, oor);
-            hot |= oor && (k > 0 || lane > 0);
+            face_fast<EXACT>(P, s_tab, WR, FR2, oor2);
+            hot |= (oor1 && cnt1) || (oor2 && cnt2);
             rfr[0 * RING + sw] = make_double2(FR2.r1, FR2.r2); rfr[1 * RING + sw] = make_double2(FR2.un, FR2.ut);
             rfr[2 * RING + sw] = make_double2(FR2.p, FR2.z1);  rfr[3 * RING + sw] = make_double2(FR2.lam, FR2.rho);
             rfr[4 * RING + sw] = make_double2(FR2.rhoE, FR2.c);
@@ -559,6 +568,7 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
     if (row < P.ny) {
         const bool redo = x_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
         if (__any_sync(0xffffffffu, redo)) {                     // rare: redo the warp's segment with the exact R13 / R17 rules
+            if ((threadIdx.x & 31) == 0) atomicAdd(&ctl->redo, 1);
             smax = 0.0; bad = 0;
             __syncwarp();
             x_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);

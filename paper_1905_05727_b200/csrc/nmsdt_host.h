@@ -66,6 +66,7 @@ void launch_diag(const Params& P, const double* q, double* partial, DiagOut* out
 void launch_derived(const Params& P, const double* q, int field_id, double* out_dense, cudaStream_t s);
 // seeded generator on the device; returns number of cavities (<0 on error); list left in d_cav
 int  generate_cavities(unsigned long long seed, double phi, double dmin, double dmax, double min_gap, int x_lo, int x_hi,
-                       int ny, int periodic_y, Cav** d_cav_out, cudaStream_t s, long long* launches);
+                       int ny, int periodic_y, Cav** d_cav_out, cudaStream_t s, long long* launches, long long* sum_r2_256,
+                       long long* target_r2_256);
 
 } // namespace nmsdt

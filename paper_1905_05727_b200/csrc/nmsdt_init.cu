@@ -360,7 +360,7 @@ __global__ void k_gen_export(int n, const long long* aX, const long long* aY, co
 }
 
 int generate_cavities(unsigned long long seed, double phi, double dmin, double dmax, double min_gap, int x_lo, int x_hi, int ny,
-                      int periodic_y, Cav** d_cav_out, cudaStream_t s, long long* launches)
+                      int periodic_y, Cav** d_cav_out, cudaStream_t s, long long* launches, long long* sum_r2_256, long long* target_r2_256)
 {
     GenPar g;
     g.seed = seed;
@@ -372,7 +372,9 @@ int generate_cavities(unsigned long long seed, double phi, double dmin, double d
     g.periodic_y = periodic_y;
     if (g.Rmin <= 0 || g.Rmax < g.Rmin || x_hi <= x_lo || ny <= 0) return -1;
     const long long target = (long long)std::floor(phi * (double)(x_hi - x_lo) * (double)ny * 65536.0 / 3.14159265358979323846);
-    const long long max_cand = 16 * (target / (g.Rmin * g.Rmin) + 1) + 1024;
+    // candidate budget (R16): 256 per cavity of the target -- the paper's densest case (phi = 8 %, centre spacing 2.5 d_c;
+    // P:153) sits close to the jamming limit of random sequential placement and needs ~40 per cavity
+    const long long max_cand = 256 * (target / (g.Rmin * g.Rmin) + 1) + 1024;
     const long long cap = target / (g.Rmin * g.Rmin) + 2;
     const int NB = 8192;
     long long *X, *Y, *R, *aX, *aY, *aR, *acc;
@@ -405,6 +407,7 @@ int generate_cavities(unsigned long long seed, double phi, double dmin, double d
         if (cudaStreamSynchronize(s) != cudaSuccess) return -2;
     }
     const int n = (int)h_acc[0];
+    *sum_r2_256 = h_acc[1]; *target_r2_256 = target;        // sum of r^2 reached / asked for, in (1/256 cell)^2
     Cav* d_cav = nullptr;
     if (cudaMalloc(&d_cav, sizeof(Cav) * (size_t)(n > 0 ? n : 1))) return -2;
     if (n > 0) { k_gen_export<<<(n + 127) / 128, 128, 0, s>>>(n, aX, aY, aR, d_cav); *launches += 1; }

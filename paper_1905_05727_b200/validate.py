@@ -22,9 +22,14 @@ PAPER_US = {("neat", 1.0, None): 4.22,
             ("random", 4.0, 0.05): 3.68, ("random", 2.0, 0.05): 3.21, ("random", 1.0, 0.05): 2.99, ("random", 1.0, 0.08): 2.67}
 
 
-def run(case, dx_um=1.0, phi=None, t_end=None, sample_every=10, seed=2019, verbose=False):
-    cfg = inputs.paper_case(case, dx_um, phi=phi, seed=seed)
+def run(case, dx_um=1.0, phi=None, t_end=None, sample_every=10, seed=2019, verbose=False, p_shock=7.81e9, length_mm=24.0,
+        limiter=None, samples=False):
+    """One validation run.  p_shock / length_mm / limiter (inputs.LIM_MINMOD, inputs.LIM_MC; R5) default to the
+    paper's case and this build's default limiter; samples=True adds the full sampled curve ("t", "M2r") to the result."""
+    cfg = inputs.paper_case(case, dx_um, p_shock=p_shock, phi=phi, seed=seed, length_mm=length_mm)
     g, ini = cfg["grid"], cfg["init"]
+    if limiter is not None:
+        g["limiter"] = int(limiter)
     if t_end is None:
         t_end = 4.8e-6 if case == "neat" else 4.4e-6
     sim = binding.Sim(g, cfg["eos"], cfg["kin"])
@@ -60,14 +65,21 @@ def run(case, dx_um=1.0, phi=None, t_end=None, sample_every=10, seed=2019, verbo
             ka = int(np.nanargmax(acc))
             if valid[0] < ka < valid[-1]:          # a maximum at the edge of the window is not a maximum
                 t_amax = float(xt[ka])
-    ncav = len(sim.cavities()) if case != "neat" else 0
+    cav = sim.cavities() if case != "neat" else np.zeros((0, 3))
+    ncav = len(cav)
+    # air fraction actually placed (a generator that ran out of candidates used to return a thinner field silently;
+    # sim_init now fails in that case, and the achieved value is reported either way)
+    phi_placed = float(np.pi * np.sum(cav[:, 2] ** 2) / ((g["nx"] - ini["shock_cells"]) * g["ny"])) if ncav else 0.0
     sim.close()
     key = (case, float(dx_um), None if case == "neat" else (phi if phi is not None else (0.08 if case == "regular" else 0.05)))
-    out = {"case": cfg["name"], "grid": [g["nx"], g["ny"]], "dx_um": dx_um, "phi": key[2], "cavities": ncav, "steps": steps,
+    out = {"case": cfg["name"], "grid": [g["nx"], g["ny"]], "dx_um": dx_um, "phi": key[2], "phi_placed": phi_placed, "cavities": ncav,
+           "limiter": "MC" if g["limiter"] == inputs.LIM_MC else "minmod", "p_shock": p_shock, "steps": steps,
            "t_final_us": float(d["t"]) * 1e6, "overtake_us": float(tm[k]) * 1e6, "peak_rate_per_s": float(rate[k]),
            "t_max_shock_acceleration_us": None if t_amax is None else t_amax * 1e6,
-           "paper_overtake_us": PAPER_US.get(key), "bad_state": int(d["bad_state"]), "wall_s": wall,
+           "paper_overtake_us": PAPER_US.get(key) if (p_shock == 7.81e9 and length_mm == 24.0) else None, "bad_state": int(d["bad_state"]), "wall_s": wall,
            "gcell_updates_per_s": g["nx"] * g["ny"] * steps / wall / 1e9}
+    if samples:
+        out["t"], out["M2r"], out["M2tot0"] = ts, M, float(d["M2tot0"])
     if verbose:
         out["curve_t_us"] = (tm[::20] * 1e6).round(4).tolist()
         out["curve_rate"] = rate[::20].tolist()
@@ -82,8 +94,12 @@ def main():
     ap.add_argument("--t-end", type=float, default=None)
     ap.add_argument("--seed", type=int, default=2019)
     ap.add_argument("--curve", action="store_true")
+    ap.add_argument("--limiter", default=None, choices=["minmod", "mc"], help="slope limiter (DESIGN.md R5); default: the build's default")
+    ap.add_argument("--p-shock", type=float, default=7.81e9)
+    ap.add_argument("--length-mm", type=float, default=24.0)
     a = ap.parse_args()
-    print(json.dumps(run(a.case, a.dx, a.phi, a.t_end, seed=a.seed, verbose=a.curve)))
+    lim = None if a.limiter is None else (inputs.LIM_MC if a.limiter == "mc" else inputs.LIM_MINMOD)
+    print(json.dumps(run(a.case, a.dx, a.phi, a.t_end, seed=a.seed, verbose=a.curve, p_shock=a.p_shock, length_mm=a.length_mm, limiter=lim)))
 
 
 if __name__ == "__main__":

@@ -31,3 +31,10 @@ def l1_rel(qa, qb):
         den = mom if k in (2, 3) else float(np.sum(np.abs(qb[k])))
         out.append(float(np.sum(np.abs(qa[k] - qb[k])) / (den if den > 0 else 1.0)))
     return out
+
+
+def rate_curve(t, M2r, M2tot0):
+    """Eq. 12-13 on samples (R14): |dM2r/dt| / M2tot0 by backward differences between consecutive samples,
+    assigned to the mid time.  Returns (t_mid, rate)."""
+    t, M2r = np.asarray(t, dtype=np.float64), np.asarray(M2r, dtype=np.float64)
+    return 0.5 * (t[1:] + t[:-1]), np.abs(np.diff(M2r)) / np.diff(t) / M2tot0

@@ -302,6 +302,81 @@ def test_rare_paths_density_outside_the_power_tables(O, B, patch):
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
+def test_rare_paths_reactant_mass_outside_its_bounds(O, B, variant):
+    """O3 clamps lambda = q6/q1 to [0, 1] and O5 moves q1 Q (lambda_0 - lambda_1) with that clamped lambda_0.  Cells planted
+    with q6 > q1 and with q6 < 0 (in the hot wake, where the source step is active, and in cold liquid) must come out of the
+    leading source step (fused: applied on load, pass 1) as the oracle's do; after the step every lambda is inside again."""
+    cfg, o = _developed_c1(O, reactive=1, steps=400)
+    q = o.state()
+    rng = np.random.default_rng(5)
+    for (j0, i0) in ((20, 10), (64, 20), (100, 60), (64, 200), (5, 250)):
+        for j in range(j0, j0 + 4):
+            for i in range(i0, i0 + 4):
+                f = rng.choice([1.0 + 1e-3, 1.2, -1e-3, -0.3, 1.0 + 1e-15])
+                q[6][j, i] = f * q[1][j, i]
+    o2, s = _pair(O, B, cfg, variant=variant)
+    o2.init_fields(q)
+    _sync_state(o2, s)
+    for it in range(2):
+        o2.step(1), s.step(1)
+        _assert_one_step(o2, s, tol=(it + 1) * TOL_ONE_STEP, what="planted q6, step %d" % it)
+    assert s.diagnostics()["bad_state"] == 0
+    lam = o2.read_field("lambda")
+    assert lam.min() >= 0.0 and lam.max() <= 1.0
+
+
+@pytest.mark.parametrize("nx,ny", [(255, 64), (257, 31), (4093, 8), (2051, 5)])
+def test_odd_nx_takes_the_fast_path(O, B, nx, ny):
+    """Rows with an odd number of cells end in a pair whose second cell is row padding: the x-sweep must neither store nor
+    act on what it computes from it (no redo of the row's last segment), and still match the oracle."""
+    cfg = inputs.config("C4", nx=nx, ny=ny, p_shock=9e9)
+    o, s = _pair(O, B, cfg, variant=1)
+    o.init(cfg["init"])
+    o.step(60)
+    _sync_state(o, s)
+    for it in range(4):
+        o.step(1), s.step(1)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="odd nx %d step %d" % (nx, it))
+    assert s.redo_count() == 0
+    # ... while a run that needs the exact rules does count (theta_0 lowered: every shocked cell sub-steps)
+    cfg["kin"]["substep_theta"] = 2e-5
+    s2 = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=1)
+    s2.init_fields(o.state())
+    s2.step(1)
+    assert s2.redo_count() > 0
+
+
+def test_generator_reports_the_air_fraction_it_placed(O, B):
+    """R16: the seeded generator stops at the target air fraction; a target at the jamming limit of the minimum gap is an
+    error, not a silently thinner field (the paper's densest case, phi = 8 % with centre spacing 2.5 d_c, is
+    reachable and must be reached)"""
+    cfg = inputs.paper_case("random", dx_um=8.0, phi=0.08)
+    g, ini = cfg["grid"], cfg["init"]
+    s = B.Sim(g, cfg["eos"], cfg["kin"])
+    s.init(ini)
+    want, got = s.cavity_stats()
+    cav = s.cavities()
+    area = (ini["x_hi"] - ini["x_lo"]) * g["ny"]
+    assert want == 0.08 and got >= 0.08 and got == pytest.approx(np.pi * np.sum(cav[:, 2] ** 2) / area, rel=1e-12)
+    assert got - 0.08 < np.pi * cav[0, 2] ** 2 / area                  # stops with the cavity that reaches the target
+    ref = O.gen_cavities(ini["seed"], ini["phi"], ini["dmin"], ini["dmax"], ini["min_gap"], ini["x_lo"], ini["x_hi"], g["ny"], 1)
+    assert np.array_equal(cav, ref)
+    # Eq. 8 (P:139): N = 4 phi L W / (pi d_c^2)
+    assert len(cav) == int(np.ceil(4 * 0.08 * area / (np.pi * ini["dmin"] ** 2)))
+    ini_bad = dict(ini, phi=0.12)                                       # exclusion disks would cover 0.75 of the plane: beyond jamming
+    with pytest.raises(B.NmsdtError) as e:
+        s.init(ini_bad)
+    assert e.value.code == B.SIM_ERR_ARG and "air fraction" in str(e.value)
+    want, got = s.cavity_stats()
+    assert want == 0.12 and 0.08 < got < 0.10
+    with pytest.raises(B.NmsdtError):
+        s.step(1)                                                       # the failed init left no usable state
+    s.init(ini)
+    s.step(2)
+    assert s.diagnostics()["bad_state"] == 0
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("d", [0, 1])
 def test_rare_paths_first_order_fallback(O, B, d, variant):
     """R17: the scheme never needs the fallback at CFL 0.4 (nor at 10x that step); a sweep with 40x (x) / 160x (y) the

@@ -1,0 +1,79 @@
+"""SURVEY 8(f) NEXT-2 under test: `validate.run` (the paper-scale validation driver, Tables IV-V) on
+rungs the oracle can afford, against the oracle driven on the same `inputs.paper_case` with the same sampling rule:
+overtake time (time of the peak of the global reaction rate, Eq. 12-13) and the sampled curve within 0.5 %.
+
+  * neat NM, 7.81 GPa, 24 mm at dx = 16 um (1500 x 32) -- the rung tests/test_oracle_sdt.py pins to the paper's 4.22 us;
+  * regular cavity array (Eq. 7: one row of d_c = 100 um cavities in a strip of width delta_c, phi = 8 %), dx = 8 um,
+    12 mm, 9.4 GPa so that hot-spot ignition and the overtake fall inside what the oracle finishes in seconds.
+The paper-scale tables themselves (dx = 1 um: 24000 x 313, 24000 x 2000) are builder-run context in profiles/.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1905_05727_b200 import inputs
+from parity_util import TOL_RATE, rate_curve
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+
+@pytest.fixture(scope="module")
+def V():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1905_05727_b200 import binding, build, validate
+    build.build()
+    binding.load_library()
+    return validate
+
+
+def _oracle_leg(O, cfg, t_end, sample_every=10):
+    """the loop of validate.run, on the oracle"""
+    g, ini = cfg["grid"], cfg["init"]
+    o = O.Oracle(g, cfg["eos"], cfg["kin"], threads=os.cpu_count() or 1)
+    o.init(ini)
+    d = o.diagnostics()
+    ts, M = [0.0], [d["M2r"]]
+    steps, x_stop = 0, (g["nx"] - 64) * g["dx"]
+    while d["t"] < t_end:
+        o.step(sample_every)
+        steps += sample_every
+        d = o.diagnostics()
+        ts.append(d["t"]); M.append(d["M2r"])
+        if steps % (10 * sample_every) == 0 and o.profiles(1.01 * ini["p0"])[3] >= x_stop:
+            break
+    assert o.fallback_count() == 0
+    return np.array(ts), np.array(M), d["M2tot0"], o
+
+
+@pytest.mark.parametrize("case,kw,t_end,window_us", [
+    ("neat", dict(dx_um=16.0), 4.8e-6, (3.9, 4.3)),
+    ("regular", dict(dx_um=8.0, p_shock=9.4e9, length_mm=12.0), 1.9e-6, (1.2, 1.8)),
+])
+def test_validate_run_against_the_oracle(O, V, case, kw, t_end, window_us):
+    out = V.run(case, t_end=t_end, samples=True, **kw)
+    cfg = inputs.paper_case(case, kw["dx_um"], p_shock=kw.get("p_shock", 7.81e9), length_mm=kw.get("length_mm", 24.0))
+    tb, Mb, M0b, o = _oracle_leg(O, cfg, t_end)
+    ta, Ma, M0a = out["t"], out["M2r"], out["M2tot0"]
+    assert out["bad_state"] == 0 and out["grid"] == [cfg["grid"]["nx"], cfg["grid"]["ny"]]
+    assert M0a == pytest.approx(M0b, rel=1e-11)
+    n = min(len(ta), len(tb))
+    assert abs(len(ta) - len(tb)) <= 1                 # same stopping rule; a last sample may differ when t lands on t_end
+    np.testing.assert_allclose(ta[:n], tb[:n], rtol=1e-8)
+    tma, ra = rate_curve(ta[:n], Ma[:n], M0a)
+    tmb, rb = rate_curve(tb[:n], Mb[:n], M0b)
+    k = int(np.argmax(rb))
+    assert 10 < k < len(rb) - 10, "the peak must lie inside the run"
+    sig = rb > 0.01 * rb[k]
+    assert np.max(np.abs(ra[sig] / rb[sig] - 1.0)) < TOL_RATE
+    t_ov = tmb[k] * 1e6
+    assert out["overtake_us"] == pytest.approx(t_ov, rel=TOL_RATE)
+    assert out["peak_rate_per_s"] == pytest.approx(rb[k], rel=TOL_RATE)
+    assert window_us[0] < t_ov < window_us[1], t_ov
+    if case == "neat":
+        # the paper's number for this case, 4.22 us at dx = 1 um: within 5 % on this coarse rung (tests/test_oracle_sdt.py)
+        assert out["paper_overtake_us"] == 4.22 and abs(out["overtake_us"] / 4.22 - 1.0) < 0.05
+    else:
+        assert out["cavities"] == len(o.cavities()) > 20 and 0.07 < out["phi_placed"] < 0.09
+    print("%s: overtake %.4f us (oracle %.4f), peak %.3e /s, %d steps" % (out["case"], out["overtake_us"], t_ov, rb[k], out["steps"]))
