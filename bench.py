@@ -210,6 +210,8 @@ def main():
     ap.add_argument("--no-slab", action="store_true")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"])
     ap.add_argument("--transport", default="staged", choices=["staged", "peer"])
+    ap.add_argument("--no-graph", action="store_true", help="A/B: enqueue every kernel instead of replaying step pairs as a CUDA graph")
+    ap.add_argument("--no-pdl", action="store_true", help="A/B: plain stream order instead of programmatic dependent launch")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -239,6 +241,7 @@ def main():
     g = cfg["grid"]
     cells = g["nx"] * g["ny"]
     sim = binding.Sim(g, cfg["eos"], cfg["kin"], variant=args.variant)
+    sim.set_launch_mode(use_graph=not args.no_graph, use_pdl=not args.no_pdl)
     sim.init(cfg["init"])
     ncav = len(sim.cavities())
 

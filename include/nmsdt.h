@@ -218,6 +218,10 @@ int sim_slab_ipc_close(void* device_base);
 
 /* Select kernel variant (SIM_VARIANT_*) and whether sim_step replays CUDA graphs (default on). */
 int sim_set_variant(sim_t*, int variant, int use_graph);
+/* How sim_step enqueues the fused variant's kernels (5 per step): use_graph = pairs of steps replayed as one CUDA graph,
+   use_pdl = the kernels chained by programmatic dependent launch (a kernel's prologue overlaps its predecessor's tail).
+   Both on by default; they change when kernels start, never what they compute (measured A/B: BASELINE.md). */
+int sim_set_launch_mode(sim_t*, int use_graph, int use_pdl);
 /* Number of kernel launches enqueued by this handle so far (bench.py's gpu_launches). */
 long long sim_launch_count(const sim_t*);
 /* Device pointer / layout of plane k of the current state (for zero-copy consumers). */
@@ -231,6 +235,12 @@ int sim_profile(sim_t*, int on);
 int sim_kernel_time(const sim_t*, int kind, double* ms_total, long long* launches);
 /* Measured FP64 FMA throughput of this device in GFLOP/s (2 flop per DFMA), probe kernel of ~ms. [sync] */
 int sim_probe_fp64(sim_t*, double* gflops_out, double* ms_out);
+/* Issue-slot probe behind the roofline model of DESIGN.md section 6: times [ms] of a kernel of 8 independent DFMA chains
+   per thread with 0, 4, 8 and 16 independent 32-bit ALU instructions interleaved per 8 DFMA, at the sweeps' residency
+   (4 warps per scheduler).  ms_out[k]/ms_out[0] = 1, 1, 1, 1.5 would mean the other instructions hide under the
+   half-rate FP64 pipe; 1, 1.25, 1.5, 2 means a DFMA holds the issue port for both of its cycles, so that a step
+   costs 2 F + O issue slots (F FP64-pipe instructions, O others). [sync] */
+int sim_probe_issue(sim_t*, double ms_out[4]);
 /* Accuracy probe of the fused path's own fp64 elementary functions (the Cochran-Chan powers of Eq. 3-4, and
    the Arrhenius exponential of Eq. 6, are evaluated with these instead of the CUDA math library; DESIGN.md
    section 5).  Evaluates function `fn` on host_x[n] on the device and returns host_y0[n], host_y1[n] (HOST arrays,

@@ -21,8 +21,8 @@ FIELD = {"q0": 0, "q1": 1, "q2": 2, "q3": 3, "q4": 4, "q5": 5, "q6": 6, "p": 16,
 # every symbol include/nmsdt.h declares (tests check that the library exports each one)
 SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error", "sim_init", "sim_init_fields",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
-           "sim_read_field", "sim_get_cavities", "sim_cavity_stats", "sim_redo_count", "sim_set_variant", "sim_launch_count", "sim_device_layout",
-           "sim_probe_fp64", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
+           "sim_read_field", "sim_get_cavities", "sim_cavity_stats", "sim_redo_count", "sim_set_variant", "sim_set_launch_mode", "sim_launch_count", "sim_device_layout",
+           "sim_probe_fp64", "sim_probe_issue", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
            "sim_shock_kinematics", "sim_init_slab", "sim_slab_halo_bytes", "sim_slab_begin", "sim_slab_smax_ptr",
            "sim_slab_ctl", "sim_slab_pass_dir", "sim_slab_pass", "sim_slab_pack", "sim_slab_unpack", "sim_slab_info",
            "sim_slab_connect", "sim_slab_push", "sim_slab_ipc_export", "sim_slab_ipc_open", "sim_slab_ipc_close"]
@@ -108,10 +108,12 @@ def load_library():
         "sim_cavity_stats": (C.c_int, [vp, dp, dp]),
         "sim_redo_count": (C.c_int, [vp, C.POINTER(C.c_longlong)]),
         "sim_set_variant": (C.c_int, [vp, C.c_int, C.c_int]),
+        "sim_set_launch_mode": (C.c_int, [vp, C.c_int, C.c_int]),
         "sim_launch_count": (C.c_longlong, [vp]),
         "sim_device_layout": (C.c_int, [vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(C.c_int),
                                         C.POINTER(C.c_int), C.POINTER(C.c_int)]),
         "sim_probe_fp64": (C.c_int, [vp, dp, dp]),
+        "sim_probe_issue": (C.c_int, [vp, dp]),
         "sim_profiles": (C.c_int, [vp, C.c_double, dp, dp, dp, dp]),
         "sim_qdot_pdf": (C.c_int, [vp, C.c_double, C.c_double, C.c_int, dp, C.POINTER(C.c_longlong)]),
         "sim_shock_kinematics": (C.c_int, [vp, dp, dp, C.c_int, C.c_double, dp, dp]),
@@ -282,6 +284,9 @@ class Sim:
     def set_variant(self, variant, use_graph=True):
         self._chk(self.L.sim_set_variant(self.h, int(variant), int(bool(use_graph))), "sim_set_variant")
 
+    def set_launch_mode(self, use_graph=True, use_pdl=True):
+        self._chk(self.L.sim_set_launch_mode(self.h, int(bool(use_graph)), int(bool(use_pdl))), "sim_set_launch_mode")
+
     def launch_count(self):
         return int(self.L.sim_launch_count(self.h))
 
@@ -289,6 +294,12 @@ class Sim:
         g, ms = C.c_double(), C.c_double()
         self._chk(self.L.sim_probe_fp64(self.h, C.byref(g), C.byref(ms)), "sim_probe_fp64")
         return g.value, ms.value
+
+    def probe_issue(self):
+        """times [ms] of the DFMA + M other instructions probe for M = 0, 4, 8, 16 per 8 DFMA"""
+        ms = (C.c_double * 4)()
+        self._chk(self.L.sim_probe_issue(self.h, ms), "sim_probe_issue")
+        return [ms[i] for i in range(4)]
 
     def profiles(self, p_front):
         """Eq. 9-11 and the Appendix C front position: (pbar[nx], rhobar[nx], ubar[nx], x_s)"""

@@ -70,6 +70,7 @@ struct sim {
     double phi_target = 0.0, phi_achieved = 0.0;    // seeded generator: air fraction asked for / placed (0 without a generator)
     int variant = SIM_VARIANT_FUSED;
     int use_graph = 1;
+    int use_pdl = 1;                // the step's five kernels are chained by programmatic dependent launch
     cudaGraphExec_t gexec = nullptr;    // fused path: one even (X-Y) + one odd (Y-X) step = 10 kernel nodes
     cudaStream_t cap_stream = nullptr;  // private stream the graph is captured on (the caller's may be the legacy stream)
     bool graph_failed = false;
@@ -77,6 +78,7 @@ struct sim {
     double dt_mode = -1.0;          // dt_fixed the control block was last prepared for
     long long launches = 0;
     std::string err;
+    CUtensorMap tmA, tmB;           // the two plane sets as {pitch, rows, 7} tensors with a {32, 1, 7} box (y-sweep staging)
     sim_slab_peer_t peer[2];        // slab decomposition: connected neighbours (peer-store transport)
     bool peer_on[2] = {false, false};
     // event profiling (sim_profile)
@@ -193,6 +195,30 @@ bool hugoniot(const sim_eos_t& e, double p0, double rho1_0, double rho2_0, doubl
     return true;
 }
 
+// Tensor map of one plane set for the y-sweep's bulk row copies: fp64 tensor {pitch, rows, 7 planes} (x fastest), box
+// {32 columns, 1 row, 7 planes}, no swizzle, out-of-range columns read as zero.  The encoder lives in the driver library;
+// it is fetched through the runtime so that libnmsdt.so links against nothing but libcudart.
+bool make_plane_tensor_map(CUtensorMap* tm, const double* plane0, int pitch, int rows, long long fstride)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
+            cudaGetLastError();
+            return false;
+        }
+        encode = (encode_fn)fn;
+    }
+    const cuuint64_t dims[3] = {(cuuint64_t)pitch, (cuuint64_t)rows, 7};
+    const cuuint64_t strides[2] = {(cuuint64_t)pitch * sizeof(double), (cuuint64_t)fstride * sizeof(double)};     // bytes, dims 1 and 2
+    const cuuint32_t box[3] = {32, 1, 7}, estr[3] = {1, 1, 1};
+    return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)plane0, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // event pair around one kernel launch while profiling
 struct KTimer {
     sim* s; int idx = -1;
@@ -239,11 +265,12 @@ void enqueue_step_fused(sim* s)
     const Params& P = s->P;
     const double* dtp = &s->ctl->dt;
     const int d1 = (s->host_step & 1) ? 1 : 0, d2 = 1 - d1;
-    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->A, s->inflow, d1, st); }
-    { KTimer t(s, d1 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->A, s->B, dtp, s->ctl, d1, 1, st); }
-    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->B, s->inflow, d2, st); }
-    { KTimer t(s, d2 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->B, s->A, dtp, s->ctl, d2, 2, st); }
-    { KTimer t(s, SIM_K_CFL); launch_ctl(P, s->ctl, 1, st); }
+    const bool pdl = s->use_pdl && !s->profile;      // (event pairs between the kernels would serialise them anyway)
+    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->A, s->inflow, d1, st, pdl); }
+    { KTimer t(s, d1 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->A, &s->tmA, s->B, dtp, s->ctl, d1, 1, st, pdl); }
+    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->B, s->inflow, d2, st, pdl); }
+    { KTimer t(s, d2 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->B, &s->tmB, s->A, dtp, s->ctl, d2, 2, st, pdl); }
+    { KTimer t(s, SIM_K_CFL); launch_ctl(P, s->ctl, 1, st, pdl); }
     s->launches += 5;
     s->host_step++;
 }
@@ -343,6 +370,11 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     s->scratch = (double*)(s->base + s->L.off_scratch);
     s->tab = (double*)(s->base + s->L.off_tab);
     fill_params(s);
+    if (!make_plane_tensor_map(&s->tmA, s->A, s->L.pitch, s->L.rows, s->L.fstride) || !make_plane_tensor_map(&s->tmB, s->B, s->L.pitch, s->L.rows, s->L.fstride)) {
+        if (s->owns) cudaFree(s->base);
+        delete s;
+        return fail(nullptr, SIM_ERR_CUDA, "sim_create: cuTensorMapEncodeTiled failed (the y-sweep stages its rows with bulk tensor copies)");
+    }
     init_fused_kernels();
     cudaMemsetAsync(s->base, 0, s->L.total, s->stream);
     {
@@ -510,7 +542,7 @@ int sim_sweep(sim_t* s, int dir, double dt)
     launch_set_double(s->scratch, dt, s->stream);
     launch_set_double(s->scratch + 1, 1e300, s->stream);
     launch_halo(s->P, s->A, s->inflow, dir, s->stream);
-    if (s->variant == SIM_VARIANT_FUSED) launch_sweep_fused(s->P, s->A, s->B, s->scratch, s->ctl, dir, 0, s->stream);
+    if (s->variant == SIM_VARIANT_FUSED) launch_sweep_fused(s->P, s->A, &s->tmA, s->B, s->scratch, s->ctl, dir, 0, s->stream);
     else launch_sweep_march(s->P, s->A, s->B, s->scratch, dir, s->stream);
     s->launches += 4;
     // keep the state in A: copy the interior planes back (parity-test helper, not on the hot path)
@@ -611,6 +643,15 @@ int sim_set_variant(sim_t* s, int variant, int use_graph)
     return SIM_OK;
 }
 
+int sim_set_launch_mode(sim_t* s, int use_graph, int use_pdl)
+{
+    if (!s) return SIM_ERR_ARG;
+    const int g = use_graph ? 1 : 0, p = use_pdl ? 1 : 0;
+    if (p != s->use_pdl && s->gexec) { cudaStreamSynchronize(s->stream); cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; s->graph_failed = false; }
+    s->use_graph = g; s->use_pdl = p;
+    return SIM_OK;
+}
+
 long long sim_launch_count(const sim_t* s) { return s ? s->launches : 0; }
 
 int sim_device_layout(const sim_t* s, void** plane0, long long* plane_stride, int* pitch, int* x_offset, int* y_offset)
@@ -688,7 +729,7 @@ int sim_slab_pass(sim_t* s, int pass)
     const int d = slab_dir(s, pass);
     double *in = slab_pass_input(s, pass), *out = pass == 1 ? s->B : s->A;
     { KTimer t(s, SIM_K_HALO); launch_halo(s->P, in, s->inflow, d, s->stream); }
-    { KTimer t(s, d == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(s->P, in, out, &s->ctl->dt, s->ctl, d, pass, s->stream); }
+    { KTimer t(s, d == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(s->P, in, pass == 1 ? &s->tmA : &s->tmB, out, &s->ctl->dt, s->ctl, d, pass, s->stream); }
     s->launches += 2;
     return check_cuda(s, "sim_slab_pass");
 }
@@ -808,6 +849,13 @@ int sim_probe_fp64(sim_t* s, double* gflops_out, double* ms_out)
     if (!s || !gflops_out || !ms_out) return fail(s, SIM_ERR_ARG, "sim_probe_fp64: NULL argument");
     int rc = launch_probe_fp64(s->stream, gflops_out, ms_out);
     if (rc) return fail(s, SIM_ERR_CUDA, "sim_probe_fp64 failed");
+    return SIM_OK;
+}
+
+int sim_probe_issue(sim_t* s, double ms_out[4])
+{
+    if (!s || !ms_out) return fail(s, SIM_ERR_ARG, "sim_probe_issue: NULL argument");
+    if (launch_probe_issue(s->stream, ms_out)) return fail(s, SIM_ERR_CUDA, "sim_probe_issue failed");
     return SIM_OK;
 }
 

@@ -47,6 +47,14 @@ struct Ctl {
     int redo;                     // fused path: warp segments repeated with the exact rules since sim_init (R13 / R17 / power tables)
 };
 
+// Programmatic dependent launch (the step's kernels are chained with it, nmsdt_capi.cu): a kernel lets the next one in the
+// stream be scheduled as its own blocks drain, and waits for the previous one to have completed (memory visible) before
+// it touches the state or the control block.  Everything before pdl_wait() -- table copy to shared memory, barrier
+// initialisation -- overlaps the predecessor's tail.  Every kernel of the chain calls pdl_wait(), so completion stays
+// transitive.  Both are no-ops in a kernel that was launched without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ double clampd(double x, double lo, double hi) { return x < lo ? lo : (x > hi ? hi : x); }
 
 // x^C and x^D from one logarithm

@@ -9,14 +9,16 @@
 // functions of nmsdt_math.cuh; a warp whose segment holds a cell that needs one of the rare rules (RK4 sub-steps R13,
 // first-order fallback R17, a density outside the power tables) repeats the segment with the exact rules.
 //
-//   k_ysweep: a thread owns a column and marches along y; the primitive window and the previous right-face state live in
-//             thread-private shared-memory slots (value pairs, 128-bit accesses), the half-finished update of the previous
-//             cell in registers; every load/store is a coalesced 256-byte row piece and nothing is recomputed (4 ramp-up
-//             rows per segment).
+//   k_ysweep: a thread owns a column and marches along y; a warp's next input row (32 columns x 7 planes) is staged by
+//             one bulk tensor copy (TMA, mbarrier-signalled) two rows ahead; the primitive window and the previous
+//             right-face state live in thread-private shared-memory slots (value pairs, 128-bit accesses), the
+//             half-finished update of the previous cell in registers; every load/store is a coalesced 256-byte row piece
+//             and nothing is recomputed (4 ramp-up rows per segment).
 //   k_xsweep: a warp owns a row segment and marches along x in chunks of 64 cells, 2 adjacent cells per lane
 //             (128-bit loads/stores).  Neighbour primitives, the right-face state and the face flux cross lanes through
 //             three 33-slot rings of value pairs in shared memory (slot = lane counter mod 33, so lane 31's entry of the previous
 //             chunk is lane 0's left neighbour: no halo recomputation, no copies); 3 __syncwarp per chunk.
+#include <cuda.h>           // CUtensorMap (type only: the encoder is fetched from the driver at run time, nmsdt_capi.cu)
 #include "nmsdt_host.h"
 #include "nmsdt_fast.cuh"
 
@@ -219,13 +221,8 @@ constexpr int XS_DOUBLES = XW * (RING_DOUBLES + 7 * PRING * 2);    // dynamic pa
 } // namespace
 
 // ---------------------------------------------------------------------------------------------------------------
-// y-sweep (a5): thread per column, register marching
+// input staging: cp.async (x-sweep), bulk tensor copies + mbarriers (y-sweep)
 // ---------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void cp_async8(double* smem, const double* gmem)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem) : "memory");
-}
 __device__ __forceinline__ void cp_async16(double* smem, const double* gmem)
 {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
@@ -235,9 +232,44 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// TMA (cp.async.bulk.tensor) + mbarrier primitives of the y-sweep's input staging: one lane per warp arms the stage's
+// barrier with the byte count and issues one bulk tensor copy per row -- a {32 columns, 1 row, 7 planes} box of the
+// plane set (described by a CUtensorMap built in sim_create) -- instead of 7 cp.async + their 64-bit address
+// arithmetic in every thread.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, int bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, int parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// y-sweep (a5): thread per column, register marching
+// ---------------------------------------------------------------------------------------------------------------
 constexpr int YT = 128;      // threads (columns) per block in k_ysweep
 constexpr int YST = 3;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1 in flight
-constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part (the math tables are static)
+constexpr int YS_DOUBLES = (YST * 7 + 16 + 10) * YT + 16;       // dynamic part (+ 128 bytes of alignment slack; the math tables and the barriers are static)
+
+struct YPipe { int st, ph; };
 
 // Per-thread state that lives across rows is kept in thread-private shared-memory slots ([..][YT] layout of value pairs,
 // no barriers): the staged input rows, the primitive window (cell c-1 and its backward differences) and the previous
@@ -247,13 +279,14 @@ constexpr int YS_DOUBLES = (YST * 7 + 9 + 7 + 10) * YT;          // dynamic part
 // sub-stepping or the first-order fallback (EXACT = false only; the caller then redoes the segment with EXACT = true --
 // the pass is out of place).
 template <int MODE, bool EXACT, int LIM>
-__device__ __forceinline__ bool y_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
-                                          int seg, int col, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad)
+__device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ qout, const double* __restrict__ dtp, int seg, int col, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad,
+                                          const CUtensorMap* tm, unsigned long long* bars, unsigned wmask, YPipe& pp)
 {
-    // thread-private slots, paired so that one 128-bit access moves two values: staged input rows (3 pairs + q6), the
-    // window (W(c-1), 1/rho, rho c^2 and the 7 differences W(c-1) - W(c-2): 8 pairs), the previous right-face state (5 pairs)
-    double2 (*s_q2)[3][YT] = reinterpret_cast<double2 (*)[3][YT]>(s_dyn);
-    double (*s_q1)[YT] = reinterpret_cast<double (*)[YT]>(s_dyn + YST * 6 * YT);
+    // staged input rows: per warp YST stages of [7 planes][32 columns], each filled by one bulk tensor copy;
+    // thread-private slots, paired so that one 128-bit access moves two values: the window (W(c-1), 1/rho, rho c^2 and
+    // the 7 differences W(c-1) - W(c-2): 8 pairs), the previous right-face state (5 pairs)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double (*s_st)[7][32] = reinterpret_cast<double (*)[7][32]>(s_dyn + warp * (YST * 7 * 32));
     double2 (*s_w2)[YT] = reinterpret_cast<double2 (*)[YT]>(s_dyn + YST * 7 * YT);
     double2 (*s_r2)[YT] = reinterpret_cast<double2 (*)[YT]>(s_dyn + (YST * 7 + 16) * YT);
     constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
@@ -263,36 +296,32 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
     const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
     const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
     const long long fs = P.fstride, pitch = P.pitch;
-    // field order of the sweep: normal momentum = q3, tangential = q2
-    const double* g = qin + (long long)(c0 - 2 + NGY) * pitch + NGX + col;
     double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
     const int nrows = c1 - c0 + 4;
-    auto stage_row = [&](int sg, const double* gp) {      // sweep field order: q0, q1, q3 (normal), q2 (tangential), q4, q5, q6
-        double* d = reinterpret_cast<double*>(&s_q2[sg][0][tid]);
-        cp_async8(d, gp); cp_async8(d + 1, gp + fs);
-        d = reinterpret_cast<double*>(&s_q2[sg][1][tid]);
-        cp_async8(d, gp + 3 * fs); cp_async8(d + 1, gp + 2 * fs);
-        d = reinterpret_cast<double*>(&s_q2[sg][2][tid]);
-        cp_async8(d, gp + 4 * fs); cp_async8(d + 1, gp + 5 * fs);
-        cp_async8(&s_q1[sg][tid], gp + 6 * fs);
+    // one lane per warp stages a row: the {32, 1, 7} box at (first column of the warp, row, plane 0) of the input plane set
+    const int tx = NGX + col - lane;
+    int ty = c0 - 2 + NGY;
+    auto stage_row = [&](int sg) {
+        if (lane == 0) {
+            mbar_expect_tx(&bars[sg], 7 * 32 * (int)sizeof(double));
+            tma_load_3d(&s_st[sg][0][0], tm, tx, ty, 0, &bars[sg]);
+        }
+        ++ty;
     };
-    auto read_row = [&](int sg, double q[7]) {
-        const double2 a = s_q2[sg][0][tid], b = s_q2[sg][1][tid], c = s_q2[sg][2][tid];
-        q[0] = a.x; q[1] = a.y; q[2] = b.x; q[3] = b.y; q[4] = c.x; q[5] = c.y; q[6] = s_q1[sg][tid];
+    auto read_row = [&](int sg, double q[7]) {            // sweep field order: q0, q1, q3 (normal), q2 (tangential), q4, q5, q6
+        q[0] = s_st[sg][0][lane]; q[1] = s_st[sg][1][lane]; q[2] = s_st[sg][3][lane]; q[3] = s_st[sg][2][lane];
+        q[4] = s_st[sg][4][lane]; q[5] = s_st[sg][5][lane]; q[6] = s_st[sg][6][lane];
     };
-    stage_row(0, g);
-    cp_async_commit();
-    g += pitch;
+    int st = pp.st, ph = pp.ph;                   // stage of row jj and the parity of its barrier's current phase
+    stage_row(st);
     double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
-    int st = 0;                                   // stage of row jj (jj mod 3)
     for (int jj = 0; jj < nrows; ++jj) {          // row c = c0 - 2 + jj
         const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
         if (jj + 1 < nrows) {
-            stage_row(sn, g);
-            g += pitch;
+            __syncwarp(wmask);                    // every lane is done with stage sn (row jj - 2, last read in the previous iteration)
+            stage_row(sn);
         }
-        cp_async_commit();
-        cp_async_wait<1>();
+        mbar_wait(&bars[st], ph);
         FCell Wp;
         {
             double q[7];
@@ -363,27 +392,39 @@ __device__ __forceinline__ bool y_segment(const Params& P, const double* __restr
             acc[5] = fma(-dtdx * z1n, F[7], acc[5]);
         }
         st = sn;
+        ph ^= sn == 0 ? 1 : 0;
     }
-    cp_async_wait<0>();
+    pp.st = st; pp.ph = ph;                       // (a redo of the segment goes on from here: every staged row has been consumed)
     return hot;
 }
 
 template <int MODE, int LIM>
-__global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const double* __restrict__ qin,
+__global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const __grid_constant__ CUtensorMap tm,
                                                                   double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg)
 {
-    extern __shared__ __align__(16) double s_dyn[];
+    extern __shared__ __align__(16) double s_dyn_raw[];
+    // the staged rows are bulk-copy destinations and must be 128-byte aligned: the dynamic part follows the static arrays
+    // below at whatever offset their sizes leave, so it carries 128 spare bytes and starts at the next multiple of 128
+    double* s_dyn = s_dyn_raw + ((128u - (smem_u32(s_dyn_raw) & 127u)) & 127u) / sizeof(double);
     __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];     // static: table lookups address it as [idx + const]
+    __shared__ __align__(8) unsigned long long s_bar[YT / 32][YST];
+    pdl_launch_dependents();
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
+    if (threadIdx.x < (YT / 32) * YST) mbar_init(&s_bar[0][0] + threadIdx.x, 1);
+    fence_proxy_async();
     __syncthreads();
+    pdl_wait();                                                  // the state, dt and the control block belong to the previous kernel until here
     const int col = blockIdx.x * YT + threadIdx.x;
+    const unsigned wmask = __ballot_sync(0xffffffffu, col < P.nx);
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
-        const bool redo = y_segment<MODE, false, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_dyn, smax, bad);
-        if (__any_sync(__activemask(), redo)) {                  // rare: redo the warp's segment with the exact R13 / R17 rules
+        YPipe pp{0, 0};
+        unsigned long long* bars = s_bar[threadIdx.x >> 5];
+        const bool redo = y_segment<MODE, false, LIM>(P, qout, dtp, seg, col, s_tab, s_dyn, smax, bad, &tm, bars, wmask, pp);
+        if (__any_sync(wmask, redo)) {                           // rare: redo the warp's segment with the exact R13 / R17 rules
             if ((threadIdx.x & 31) == 0) atomicAdd(&ctl->redo, 1);
             smax = 0.0; bad = 0;
-            y_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, col, s_tab, s_dyn, smax, bad);
+            y_segment<MODE, true, LIM>(P, qout, dtp, seg, col, s_tab, s_dyn, smax, bad, &tm, bars, wmask, pp);
         }
     }
     if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
@@ -561,8 +602,10 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
 {
     extern __shared__ __align__(16) double s_dyn[];
     __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
+    pdl_launch_dependents();
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
     __syncthreads();
+    pdl_wait();
     const int row = blockIdx.x * XW + (threadIdx.x >> 5);
     double smax = 0.0; int bad = 0;
     if (row < P.ny) {
@@ -608,17 +651,26 @@ __host__ __device__ inline double tsafe_for(double tau, double Cpre, double Ta, 
     // Return T* such that T < T* guarantees tau C g < theta0 (1 - 1e-6); +inf when that holds for every T.
     const double target = theta0 * (1.0 - 1e-6) / (tau * Cpre);       // need g(y) < target
     if (!(tau > 0.0) || target >= 1.0) return 1e300;
-    double lo = 0.0, hi = 1.0;                                        // g(lo) >= target > g(hi)
-    while (1.0 / (1.0 + hi * (1.0 + hi * (0.5 + hi / 6.0))) >= target) hi *= 2.0;
-    for (int it = 0; it < 64; ++it) {
-        const double mid = 0.5 * (lo + hi);
-        if (1.0 / (1.0 + mid * (1.0 + mid * (0.5 + mid / 6.0))) >= target) lo = mid; else hi = mid;
+    // y* = positive root of h(y) = 1 + y + y^2/2 + y^3/6 - 1/target (h' > 0, h'' > 0 for y > 0).  Newton from
+    // y0 = cbrt(6/target), where h(y0) = 1 + y0 + y0^2/2 > 0: the iterates fall monotonically onto the root from the right,
+    // so every one of them is a safe bound (y_n >= y*  =>  Ta/y_n <= Ta/y*).  This runs in the one-thread k_ctl of every
+    // step: a dozen divisions instead of the 64 bisections it replaced (12.8 -> ~2 us per step).
+    const double r = 1.0 / target;
+    double y = cbrt(6.0 * r);
+    for (int it = 0; it < 12; ++it) {
+        const double h = 1.0 + y * (1.0 + y * (0.5 + y * (1.0 / 6.0))) - r;
+        const double dh = 1.0 + y * (1.0 + 0.5 * y);
+        const double yn = y - h / dh;
+        if (!(yn < y)) break;                                         // converged (or rounding would step back over the root)
+        y = yn;
     }
-    return Ta / hi;                                                   // T < Ta/hi  =>  y > hi  =>  g(y) < target
+    return Ta / (y * (1.0 + 1e-12));                                  // T < Ta/y  =>  Ta/T > y >= y*  =>  g < target
 }
 
 __global__ void k_ctl(const __grid_constant__ Params P, Ctl* ctl, int advance)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     if (advance) { ctl->t += ctl->dt; ctl->dt_last = ctl->dt; ctl->step += 1; }
     const double smax = __longlong_as_double((long long)ctl->smax_bits);
     const double dt = ctl->dt_fixed > 0.0 ? ctl->dt_fixed : P.cfl * P.hmin / smax;
@@ -679,29 +731,29 @@ static int num_sms()
 }
 
 template <int MODE, int LIM>
-static void x_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl,
-                     int seg)
+static void x_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, bool pdl, const Params& P, const double* qin, double* qout, const double* dtp,
+                     Ctl* ctl, int seg)
 {
     if (attr_only) cudaFuncSetAttribute(k_xsweep<MODE, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    else k_xsweep<MODE, LIM><<<grid, 32 * XW, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+    else launch_k(k_xsweep<MODE, LIM>, grid, dim3(32 * XW), sm, s, pdl, P, qin, qout, dtp, ctl, seg);
 }
 template <int MODE, int LIM>
-static void y_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl,
-                     int seg)
+static void y_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, bool pdl, const Params& P, const CUtensorMap* tm, double* qout, const double* dtp,
+                     Ctl* ctl, int seg)
 {
     if (attr_only) cudaFuncSetAttribute(k_ysweep<MODE, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    else k_ysweep<MODE, LIM><<<grid, YT, sm, s>>>(P, qin, qout, dtp, ctl, seg);
+    else launch_k(k_ysweep<MODE, LIM>, grid, dim3(YT), sm, s, pdl, P, *tm, qout, dtp, ctl, seg);
 }
 
 // dispatch on (direction, pass kind, limiter); attr_only = opt in to the dynamic shared memory instead of launching
-static void sweep_dispatch(bool attr_only, int dir, int mode, int lim, dim3 grid, cudaStream_t s, const Params& P, const double* qin, double* qout,
-                           const double* dtp, Ctl* ctl, int seg)
+static void sweep_dispatch(bool attr_only, int dir, int mode, int lim, dim3 grid, cudaStream_t s, bool pdl, const Params& P, const double* qin,
+                           const CUtensorMap* tm, double* qout, const double* dtp, Ctl* ctl, int seg)
 {
     const size_t sm = (dir == 0 ? XS_DOUBLES : YS_DOUBLES) * sizeof(double);
 #define NMSDT_CASE(D, M, L)                                                                                          \
     if (dir == D && mode == M && lim == L) {                                                                        \
-        if (D == 0) x_launch<M, L>(attr_only, grid, sm, s, P, qin, qout, dtp, ctl, seg);                          \
-        else        y_launch<M, L>(attr_only, grid, sm, s, P, qin, qout, dtp, ctl, seg);                          \
+        if (D == 0) x_launch<M, L>(attr_only, grid, sm, s, pdl, P, qin, qout, dtp, ctl, seg);                     \
+        else        y_launch<M, L>(attr_only, grid, sm, s, pdl, P, tm, qout, dtp, ctl, seg);                      \
         return;                                                                                                     \
     }
     NMSDT_CASE(0, MODE_PLAIN, 0) NMSDT_CASE(0, MODE_LEAD, 0) NMSDT_CASE(0, MODE_TRAIL, 0) NMSDT_CASE(0, MODE_TRAIL_INERT, 0)
@@ -717,24 +769,25 @@ void init_fused_kernels()
     Params P{};
     for (int dir = 0; dir < 2; ++dir)
         for (int mode = 0; mode < 4; ++mode)
-            for (int lim = 0; lim < 2; ++lim) sweep_dispatch(true, dir, mode, lim, dim3(1), nullptr, P, nullptr, nullptr, nullptr, nullptr, 0);
+            for (int lim = 0; lim < 2; ++lim) sweep_dispatch(true, dir, mode, lim, dim3(1), nullptr, false, P, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
 }
 
 // mode 0 plain, 1 leading source on load, 2 trailing source + max-wavespeed partial.  An inert run (P.reactive = 0) has
 // no source step: its pass 1 is the plain sweep and its pass 2 the sweep + wavespeed.  The limiter (R5) is a template
 // parameter so that the marching loop stays one basic block.
-void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s)
+void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* tm_in, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s,
+                        bool pdl)
 {
     if (!P.reactive) mode = mode == MODE_LEAD ? MODE_PLAIN : (mode == MODE_TRAIL ? MODE_TRAIL_INERT : mode);
     const int lim = P.limiter == 0 ? 0 : 1;
     if (dir == 0) {
         const int lines = (P.ny + XW - 1) / XW;
         const int seg = pick_seg_x(P.nx, lines, num_sms() * NMSDT_X_MINBLOCKS);
-        sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, P, qin, qout, dtp, ctl, seg);
+        sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
         const int seg = pick_seg(P.ny, 1, 128, 4, lines, num_sms() * NMSDT_Y_MINBLOCKS);
-        sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, P, qin, qout, dtp, ctl, seg);
+        sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg);
     }
 }
 
@@ -744,7 +797,7 @@ void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStrea
     k_source_fast<<<grid, 128, 0, s>>>(P, q, dtp);
 }
 
-void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s) { k_ctl<<<1, 1, 0, s>>>(P, ctl, advance); }
+void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s, bool pdl) { launch_k(k_ctl, dim3(1), dim3(1), 0, s, pdl, P, ctl, advance); }
 
 double host_tsafe(double tau, double Cpre, double Ta, double theta0) { return tsafe_for(tau, Cpre, Ta, theta0); }
 

@@ -1,5 +1,6 @@
 // nmsdt_host.h -- host-side declarations shared by the .cu files of libnmsdt.so (not part of the public ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include "nmsdt_device.cuh"
 
@@ -19,8 +20,21 @@ struct DiagOut {   // device-side result of the diagnostics reduction
 constexpr int DIAG_BLOCKS = 1184;          // 8 x 148
 constexpr int DIAG_NV = 8;                 // 7 sums + smax
 
+// kernel launch with (pdl = true) or without the programmatic-stream-serialization attribute (see pdl_wait, nmsdt_device.cuh)
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // step kernels (nmsdt_step.cu)
-void launch_halo(const Params& P, double* q, const double* inflow, int dir, cudaStream_t s);
+void launch_halo(const Params& P, double* q, const double* inflow, int dir, cudaStream_t s, bool pdl = false);
 void launch_source(const Params& P, double* q, const double* dtp, double scale, cudaStream_t s);
 void launch_sweep_march(const Params& P, const double* qin, double* qout, const double* dtp, int dir, cudaStream_t s);
 void launch_cfl(const Params& P, const double* q, Ctl* ctl, cudaStream_t s);
@@ -28,13 +42,16 @@ void launch_finalize_dt(const Params& P, Ctl* ctl, cudaStream_t s);
 void launch_advance(Ctl* ctl, cudaStream_t s);
 void launch_set_double(double* p, double v, cudaStream_t s);
 int  launch_probe_fp64(cudaStream_t s, double* gflops, double* ms);
+int  launch_probe_issue(cudaStream_t s, double ms[4]);
 
 // fused production path (nmsdt_fused.cu). dtp -> {dt (or tau for the source kernel), tsafe}; mode 0 plain, 1 leading
 // source on load, 2 trailing source + max-wavespeed partial
 void init_fused_kernels();
-void launch_sweep_fused(const Params& P, const double* qin, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s);
+// tm_in: tensor map of the plane set qin (dims {pitch, rows, 7}, box {32, 1, 7}; make_plane_tensor_map in nmsdt_capi.cu)
+void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* tm_in, double* qout, const double* dtp, Ctl* ctl, int dir, int mode,
+                        cudaStream_t s, bool pdl = false);
 void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s);
-void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s);
+void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s, bool pdl = false);
 double host_tsafe(double tau, double Cpre, double Ta, double theta0);
 int  launch_probe_math(const PowCoef& pw, const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
                        cudaStream_t s);
