@@ -33,16 +33,19 @@ from paper_1905_05727_b200 import inputs  # noqa: E402
 
 METRIC = "fp64 cell-updates/s per 2D step"
 UNIT = "cell-updates/s"
-# algorithmic FP64 work of one cell in one fused directional sweep, from ncu's counters of the
-# C5 launches (profiles/r01j_fused_c5.md) divided by the ramp-up redundancy of a segment (65/64 on C5).
-#   FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot):
-FP64_INSTR_PER_CELL = {"lead": 351.0, "trail": 413.0}       # pass 1 = S + sweep; pass 2 = sweep + S + wavespeed
-#   flops with dadd = dmul = 1, dfma = 2, dsetp = 0 (54 % of the FP64 instructions are DFMA):
-FLOP_PER_CELL = {"lead": 524.0, "trail": 617.0}
+# the algorithmic FP64 work of one cell in one fused directional sweep comes from ncu's counters of the C5
+# launches, profiles/roofline_counts.json (written by paper_1905_05727_b200/roofline_counts.py, which also records a hash of
+# the kernel sources): FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot),
+# flops with dadd = dmul = 1, dfma = 2, dsetp = 0, and the measured DRAM bytes per cell.
 FP64_LANES_PER_SM, N_SM = 64, 148
-# dram__bytes_read.sum + dram__bytes_write.sum per cell per launch from the ncu --set full capture of C5 (mean of the
-# lead and trail launches; profiles/r01j_fused_c5.md): 113.0 B (x), 112.6 B (y) against 112 B algorithmic
-TRAFFIC_BYTES_PER_CELL = {"sweep_x": 112.95, "sweep_y": 112.6}
+
+
+def load_counts():
+    """(counts, stale): per-kernel per-cell counts of the last ncu capture; stale = the kernel sources changed since"""
+    from paper_1905_05727_b200 import roofline_counts
+    with open(os.path.join(ROOT, "profiles", "roofline_counts.json")) as f:
+        c = json.load(f)
+    return c, roofline_counts.source_hash() != c["source_sha256"]
 
 
 def peaks():
@@ -208,10 +211,11 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-slab", action="store_true")
+    ap.add_argument("--no-sustained", action="store_true")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"])
     ap.add_argument("--transport", default="staged", choices=["staged", "peer"])
     ap.add_argument("--no-graph", action="store_true", help="A/B: enqueue every kernel instead of replaying step pairs as a CUDA graph")
-    ap.add_argument("--no-pdl", action="store_true", help="A/B: plain stream order instead of programmatic dependent launch")
+    ap.add_argument("--pdl", action="store_true", help="A/B: chain the step's kernels by programmatic dependent launch")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -241,7 +245,7 @@ def main():
     g = cfg["grid"]
     cells = g["nx"] * g["ny"]
     sim = binding.Sim(g, cfg["eos"], cfg["kin"], variant=args.variant)
-    sim.set_launch_mode(use_graph=not args.no_graph, use_pdl=not args.no_pdl)
+    sim.set_launch_mode(use_graph=not args.no_graph, use_pdl=args.pdl)
     sim.init(cfg["init"])
     ncav = len(sim.cavities())
 
@@ -291,24 +295,38 @@ def main():
     # (dadd = dmul = 1, dfma = 2) is given beside it.
     pk = peaks()
     clk = sampler.summary()
+    counts, counts_stale = load_counts()
+    ck = counts["kernels"]
     sm_max = pk.get("sm_max_mhz", clk.get("sm_max_mhz") or 1965.0)
     peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     dom = max(("sweep_x", "sweep_y"), key=lambda k: kt[k][0])
+    dd = "x" if dom == "sweep_x" else "y"
     dom_ms = kt[dom][0] / max(kt[dom][1], 1)
-    instr = 0.5 * (FP64_INSTR_PER_CELL["lead"] + FP64_INSTR_PER_CELL["trail"])
-    flop = 0.5 * (FLOP_PER_CELL["lead"] + FLOP_PER_CELL["trail"])
+    mean2 = lambda key, a, b: 0.5 * (ck[a][key] + ck[b][key])          # noqa: E731  (a launch of each pass kind per two steps)
+    instr = mean2("fp64_instr_per_cell", dd + "_lead", dd + "_trail")
+    flop = mean2("flop_per_cell", dd + "_lead", dd + "_trail")
     achieved = 2.0 * instr * cells / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     try:
         probe_gflops, _ = sim.probe_fp64()
+        issue_ms = sim.probe_issue()
     except Exception:
-        probe_gflops = None
-    step_instr = FP64_INSTR_PER_CELL["lead"] + FP64_INSTR_PER_CELL["trail"]
+        probe_gflops, issue_ms = None, None
+    # an even step is x-lead + y-trail, an odd one y-lead + x-trail: K steps alternate
+    step_instr = 0.5 * sum(ck[k]["fp64_instr_per_cell"] for k in ("x_lead", "x_trail", "y_lead", "y_trail"))
+    step_other = 0.5 * sum(ck[k]["warp_instr_per_cell"] for k in ("x_lead", "x_trail", "y_lead", "y_trail")) - step_instr
     roof = {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-            "frac": achieved / peak_tflops, "traffic": TRAFFIC_BYTES_PER_CELL.get(dom) * cells if args.config == "C5" else None,
-            "counting": "FP64-pipe issue slots x 2 flop (DFMA-equivalent); %.0f FP64 instr/cell/launch" % instr,
+            "frac": achieved / peak_tflops,
+            "traffic": mean2("dram_bytes_per_cell", dd + "_lead", dd + "_trail") * cells if args.config == "C5" else None,
+            "counting": "FP64-pipe issue slots x 2 flop (DFMA-equivalent); %.1f FP64 instr/cell/launch" % instr,
+            "counts_from": "profiles/roofline_counts.json (%s, %s)" % (counts["round"], counts["workload"]), "counts_stale": bool(counts_stale),
             "achieved_plain_flops": flop * cells / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0,
             "peak_source": "148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (guide's unit counts and clock)",
             "peak_measured_dfma_probe": probe_gflops / 1e3 if probe_gflops else None,
+            # the issue model behind "alu": time of 8 DFMA chains with 0 / 4 / 8 / 16 other instructions per 8 DFMA, relative to 0
+            # (1, 1.25, 1.5, 2 = a DFMA holds the issue port for both of its cycles: a step costs 2 F + O slots)
+            "issue_probe_ratio": [x / issue_ms[0] for x in issue_ms] if issue_ms else None,
+            "fp64_instr_per_cell_step": step_instr, "other_instr_per_cell_step": step_other,
+            "issue_slot_frac": ((2.0 * step_instr + step_other) * cells / 32.0 / (N_SM * 4) / (ms / K * 1e-3 * sm_max * 1e6)),
             "whole_step_frac": 2.0 * step_instr * cells * K / (ms * 1e-3) / 1e12 / peak_tflops,
             # the same against the peak at the SM clock nvidia-smi reported during the timed region (the step runs close to the
             # board's power limit: sw_power_cap lowers the clock by a few per cent on some boards)
@@ -317,7 +335,29 @@ def main():
             "ms_per_launch": dom_ms,
             "hbm_gbs_algorithmic": 112.0 * cells / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0,
             "hbm_peak_gbs": pk.get("hbm_gbs", 6650.0),
-            "kernel_ms_per_step": {k: v[0] / K for k, v in kt.items()}}
+            "kernel_ms_per_step": {k: v[0] / K for k, v in kt.items()},
+            "geometry": {"x": sim.sweep_geometry(0), "y": sim.sweep_geometry(1)}, "redo_count": sim.redo_count()}
+
+    # ---- sustained: BASELINE config 5's protocol, 20 warm-up + 200 timed steps back to back (the board reaches its power cap
+    # after about a second), with its own clock record; launched the way a user runs it (CUDA-graph replay, no event pairs)
+    sustained = None
+    if not args.no_sustained:
+        sim.step(20)
+        barrier()
+        smp = ClockSampler(local)
+        smp.start()
+        e0.record(sim.stream)
+        sim.step(200)
+        e1.record(sim.stream)
+        barrier()
+        smp.stop_flag = True
+        smp.join(timeout=2)
+        sms = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+        sc = smp.summary()
+        sustained = {"steps": 200, "warmup": 20, "ms_per_step": sms / 200, "value": aggregate_value(cells, 200, world, sms * 1e-3), "unit": UNIT,
+                     "clocks": sc, "whole_step_frac": 2.0 * step_instr * cells * 200 / (sms * 1e-3) / 1e12 / peak_tflops,
+                     "whole_step_frac_at_measured_clock": (2.0 * step_instr * cells * 200 / (sms * 1e-3) / 1e12 / peak_tflops * sm_max / sc["sm_mhz"]
+                                                           if sc.get("sm_mhz") else None)}
 
     # ---- post-processing calls (not part of a step): one state read each, HBM bound ----------------
     post = {}
@@ -385,14 +425,16 @@ def main():
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s %dx%d, %d cavities, p_shock %.3g Pa, fp64 SoA 7 planes double-buffered; replicas only; "
-                               "state %.1f MB %s" % (args.config, g["nx"], g["ny"], ncav, cfg["init"]["p_shock"], 7 * cells * 8 / 1e6,
+        "config": {"workload": "%s %dx%d, %d cavities, p_shock %.3g Pa, fp64 SoA 7 planes double-buffered; %s; "
+                               "state %.1f MB %s" % (args.config, g["nx"], g["ny"], ncav, cfg["init"]["p_shock"],
+                                  "replicas only" if world == 1 else "%d independent replicas (one per GPU: throughput of %d separate runs, NOT a scaling result of the "
+                                  "method; --decomp slab runs one domain cut into x-slabs)" % (world, world), 7 * cells * 8 / 1e6,
                                                      "> L2 (no flush needed)" if 7 * cells * 8 > 126e6 else "fits the 126 MB L2 (small config, not a bench line)"),
                    "variant": args.variant, "ranks_share_a_gpu": bool(shared_gpu), "kernel_timing": "event pairs inside the timed region" if profile_in_timed else
                    "timed region = CUDA-graph replay; kernel event pairs in a second pass", "l2_policy": "inputs larger than L2" if 7 * cells * 8 > 126e6 else "L2-resident (small config)"},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
         "sim": {"t": d["t"], "step": d["step"], "bad_state": d["bad_state"], "burned_mass": d["burned_mass"]},
-        "post": post, "slab": slab_block,
+        "post": post, "slab": slab_block, "sustained": sustained,
     }
     print(json.dumps(out))
     if world > 1:

@@ -218,10 +218,15 @@ int sim_slab_ipc_close(void* device_base);
 
 /* Select kernel variant (SIM_VARIANT_*) and whether sim_step replays CUDA graphs (default on). */
 int sim_set_variant(sim_t*, int variant, int use_graph);
-/* How sim_step enqueues the fused variant's kernels (5 per step): use_graph = pairs of steps replayed as one CUDA graph,
-   use_pdl = the kernels chained by programmatic dependent launch (a kernel's prologue overlaps its predecessor's tail).
-   Both on by default; they change when kernels start, never what they compute (measured A/B: BASELINE.md). */
+/* How sim_step enqueues the fused variant's kernels (5 per step): use_graph = pairs of steps replayed as one CUDA graph
+   (default on), use_pdl = the kernels chained by programmatic dependent launch, a kernel's prologue overlapping its
+   predecessor's tail (default off: measured 3-6 % slower than plain graph edges on the launch-bound configs, equal on
+   the large ones).  They change when kernels start, never what they compute. */
 int sim_set_launch_mode(sim_t*, int use_graph, int use_pdl);
+/* Launch geometry of the fused sweep in direction dir (0 = x, 1 = y) on this grid: a block (y: 128 columns, x: 4 rows)
+   marches over *seg cells after *ramp recomputed ramp-up cells; *nblocks blocks per launch.  The kernels execute
+   (seg + ramp)/seg times the algorithmic work: the roofline block of bench.py divides that out. */
+int sim_sweep_geometry(const sim_t*, int dir, int* seg, int* ramp, long long* nblocks);
 /* Number of kernel launches enqueued by this handle so far (bench.py's gpu_launches). */
 long long sim_launch_count(const sim_t*);
 /* Device pointer / layout of plane k of the current state (for zero-copy consumers). */

@@ -14,13 +14,19 @@ HDR = [os.path.join(HERE, "nmsdt_oracle.h")]
 
 
 def build(force: bool = False) -> str:
-    deps = SRC + HDR
-    if (not force) and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
-        return LIB
-    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
-           "-Wall", "-Wextra", "-o", LIB] + SRC
+    """ORACLE_SANITIZE=1 builds and returns liboracle_san.so instead: the same source under AddressSanitizer and
+    UndefinedBehaviorSanitizer (run python with LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0;
+    profiles/r02_sanitizers.md)."""
+    san = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+    lib = os.path.join(HERE, "liboracle_san.so") if san else LIB
+    deps = SRC + HDR + [os.path.abspath(__file__)]
+    if (not force) and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in deps):
+        return lib
+    opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] if san else ["-O2"]
+    cmd = ["g++", "-std=c++17"] + opt + ["-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
+                                         "-Wall", "-Wextra", "-o", lib] + SRC
     subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

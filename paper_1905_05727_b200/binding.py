@@ -21,7 +21,7 @@ FIELD = {"q0": 0, "q1": 1, "q2": 2, "q3": 3, "q4": 4, "q5": 5, "q6": 6, "p": 16,
 # every symbol include/nmsdt.h declares (tests check that the library exports each one)
 SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error", "sim_init", "sim_init_fields",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
-           "sim_read_field", "sim_get_cavities", "sim_cavity_stats", "sim_redo_count", "sim_set_variant", "sim_set_launch_mode", "sim_launch_count", "sim_device_layout",
+           "sim_read_field", "sim_get_cavities", "sim_cavity_stats", "sim_redo_count", "sim_set_variant", "sim_set_launch_mode", "sim_sweep_geometry", "sim_launch_count", "sim_device_layout",
            "sim_probe_fp64", "sim_probe_issue", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
            "sim_shock_kinematics", "sim_init_slab", "sim_slab_halo_bytes", "sim_slab_begin", "sim_slab_smax_ptr",
            "sim_slab_ctl", "sim_slab_pass_dir", "sim_slab_pass", "sim_slab_pack", "sim_slab_unpack", "sim_slab_info",
@@ -109,6 +109,7 @@ def load_library():
         "sim_redo_count": (C.c_int, [vp, C.POINTER(C.c_longlong)]),
         "sim_set_variant": (C.c_int, [vp, C.c_int, C.c_int]),
         "sim_set_launch_mode": (C.c_int, [vp, C.c_int, C.c_int]),
+        "sim_sweep_geometry": (C.c_int, [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]),
         "sim_launch_count": (C.c_longlong, [vp]),
         "sim_device_layout": (C.c_int, [vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(C.c_int),
                                         C.POINTER(C.c_int), C.POINTER(C.c_int)]),
@@ -157,10 +158,15 @@ def workspace_bytes(grid):
     return int(load_library().sim_workspace_bytes(C.byref(_fill(Grid(), grid))))
 
 
+def workspace_bytes(grid):
+    """sim_workspace_bytes for a grid dict"""
+    return int(load_library().sim_workspace_bytes(C.byref(_fill(Grid(), grid))))
+
+
 class Sim:
     """One simulation on the current CUDA device. grid/eos/kin/init are plain dicts (see `inputs`)."""
 
-    def __init__(self, grid, eos, kin, device=None, variant=None, use_graph=True, library_workspace=False):
+    def __init__(self, grid, eos, kin, device=None, variant=None, use_graph=True, library_workspace=False, workspace=None):
         import torch
         self.L = load_library()
         if not torch.cuda.is_available():
@@ -177,7 +183,13 @@ class Sim:
         self.h = C.c_void_p()
         with torch.cuda.device(self.device):
             # device memory: torch's, unless the workspace must be a cudaMalloc allocation of its own (CUDA IPC export)
-            self.workspace = None if library_workspace else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            # (workspace: a caller's own 256-byte aligned uint8 tensor of at least sim_workspace_bytes -- e.g. one with guard bands)
+            if workspace is not None:
+                if workspace.dtype != torch.uint8 or workspace.numel() < nbytes or not workspace.is_contiguous():
+                    raise ValueError("workspace must be a contiguous uint8 CUDA tensor of at least %d bytes" % nbytes)
+                self.workspace = workspace
+            else:
+                self.workspace = None if library_workspace else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = torch.cuda.current_stream(self.device)
             rc = self.L.sim_create(C.byref(self.grid), C.byref(self.eos), C.byref(self.kin),
                                    C.c_void_p(self.workspace.data_ptr() if self.workspace is not None else None),
@@ -284,8 +296,14 @@ class Sim:
     def set_variant(self, variant, use_graph=True):
         self._chk(self.L.sim_set_variant(self.h, int(variant), int(bool(use_graph))), "sim_set_variant")
 
-    def set_launch_mode(self, use_graph=True, use_pdl=True):
+    def set_launch_mode(self, use_graph=True, use_pdl=False):
         self._chk(self.L.sim_set_launch_mode(self.h, int(bool(use_graph)), int(bool(use_pdl))), "sim_set_launch_mode")
+
+    def sweep_geometry(self, d):
+        """(segment length, ramp-up cells, blocks per launch) of the fused sweep in direction d"""
+        seg, ramp, nb = C.c_int(), C.c_int(), C.c_longlong()
+        self._chk(self.L.sim_sweep_geometry(self.h, int(d), C.byref(seg), C.byref(ramp), C.byref(nb)), "sim_sweep_geometry")
+        return seg.value, ramp.value, nb.value
 
     def launch_count(self):
         return int(self.L.sim_launch_count(self.h))

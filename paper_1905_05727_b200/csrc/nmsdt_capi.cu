@@ -70,7 +70,7 @@ struct sim {
     double phi_target = 0.0, phi_achieved = 0.0;    // seeded generator: air fraction asked for / placed (0 without a generator)
     int variant = SIM_VARIANT_FUSED;
     int use_graph = 1;
-    int use_pdl = 1;                // the step's five kernels are chained by programmatic dependent launch
+    int use_pdl = 0;                // chain the step's five kernels by programmatic dependent launch (measured slower: off)
     cudaGraphExec_t gexec = nullptr;    // fused path: one even (X-Y) + one odd (Y-X) step = 10 kernel nodes
     cudaStream_t cap_stream = nullptr;  // private stream the graph is captured on (the caller's may be the legacy stream)
     bool graph_failed = false;
@@ -640,6 +640,13 @@ int sim_set_variant(sim_t* s, int variant, int use_graph)
 {
     if (!s || (variant != SIM_VARIANT_UNFUSED && variant != SIM_VARIANT_FUSED)) return fail(s, SIM_ERR_ARG, "sim_set_variant: bad argument");
     s->variant = variant; s->use_graph = use_graph ? 1 : 0; s->cfl_valid = false;
+    return SIM_OK;
+}
+
+int sim_sweep_geometry(const sim_t* s, int dir, int* seg, int* ramp, long long* nblocks)
+{
+    if (!s || (dir != 0 && dir != 1) || !seg || !ramp || !nblocks) return SIM_ERR_ARG;
+    sweep_geometry(s->P, dir, seg, ramp, nblocks);
     return SIM_OK;
 }
 

@@ -683,38 +683,46 @@ __global__ void k_ctl(const __grid_constant__ Params P, Ctl* ctl, int advance)
 // launchers
 // ---------------------------------------------------------------------------------------------------------------
 // Segment length along the marching axis.  A block marches over `seg` cells after `ramp` cells of ramp-up (recomputed
-// halo), `lines` blocks stand side by side, and `slots` blocks are resident on the whole GPU at once, so the sweep
-// takes about ceil(lines * nseg / slots) * (seg + ramp) marching iterations: pick the nseg that minimises that
-// (large grids end up near `target`, small ones are cut into enough segments to fill all SMs).
-static int pick_seg(int n, int unit, int target, int ramp, int lines, int slots)
+// halo) and a start that costs about `start` iterations (table copy, first staged row); `lines` blocks stand side by side,
+// and up to `maxb` blocks are resident per SM.  With B = lines * nseg blocks:
+//   * B > nsm * maxb (large grids): ceil(B / (nsm maxb)) waves of (seg + ramp + start) iterations, each at the throughput-bound
+//     pace of maxb resident blocks -- large grids end up near `target`, with little ramp-up redundancy;
+//   * otherwise one wave with b = ceil(B / nsm) blocks per SM, whose iterations take max(lat, b) / maxb of that pace: a lone
+//     block is bound by the latency of the cell's dependency chain (measured: an iteration of a lone block takes lat = 2.6 (y),
+//     2.5 (x) times as long as its share of a full SM's), so small grids are cut into as many short segments as the SMs
+//     can take before throughput binds -- on a machine that is not full, recomputed ramp-up cells are free and latency counts
+//     (C1: 6 instead of 12 rows per block).
+static double seg_cost(long long B, double iters, int nsm, int maxb, double lat)
 {
-    const int max_seg = (n + unit - 1) / unit;                 // in units
-    int best_seg = max_seg * unit; double best = 1e300;
-    const int su0 = (2 * ramp + unit - 1) / unit < max_seg ? (2 * ramp + unit - 1) / unit : max_seg;   // redundancy <= 1.5
-    for (int su = su0; su <= max_seg; ++su) {
-        const int seg = su * unit;
-        if (seg > 2 * target && su > su0) break;
+    const long long b = (B + nsm - 1) / nsm;
+    if (b <= maxb) return iters * (lat > (double)b ? lat : (double)b);
+    return (double)((B + (long long)nsm * maxb - 1) / ((long long)nsm * maxb)) * iters * maxb;
+}
+
+static int pick_seg(int n, int target, int ramp, double start, int lines, int nsm, int maxb, double lat)
+{
+    int best_seg = n; double best = 1e300;
+    for (int seg = n < 2 ? n : 2; seg <= n; ++seg) {
+        if (seg > 2 * target) break;
         const int nseg = (n + seg - 1) / seg;
-        const double waves = (double)(((long long)lines * nseg + slots - 1) / slots);
-        const double cost = waves * (seg + ramp);
+        const double cost = seg_cost((long long)lines * nseg, seg + ramp + start, nsm, maxb, lat);
         if (cost < best * (1.0 - 1e-9)) { best = cost; best_seg = seg; }
     }
     return best_seg;
 }
 
 // x-sweep: a segment of 64 m - XRAMP cells takes exactly m marching iterations of 64 cells (the first chunk starts XRAMP
-// cells to the left); pick the m that minimises waves x (iterations + 2): a block's start (table copy, first staged chunk)
-// costs about two iterations.  Segment starts stay even (128-bit pair loads).
-static int pick_seg_x(int n, int lines, int slots)
+// cells to the left) after a start (table copy, first staged chunk) that costs about two iterations.  Segment starts stay
+// even (128-bit pair loads).
+static int pick_seg_x(int n, int lines, int nsm, int maxb, double lat)
 {
     const int mmax = (n + XRAMP + 63) / 64;                    // one segment for the whole row
     int best = 64 * mmax - XRAMP; double bestc = 1e300;
-    for (int m = 2; m <= mmax; ++m) {
+    for (int m = 1; m <= mmax; ++m) {
         const int seg = 64 * m - XRAMP;
         if (seg > 4096 && m < mmax) continue;                  // segments of at most a few thousand cells, or the whole row
         const int nseg = (n + seg - 1) / seg;
-        const double waves = (double)(((long long)lines * nseg + slots - 1) / slots);
-        const double cost = waves * (m + 2.0);
+        const double cost = seg_cost((long long)lines * nseg, m + 2.0, nsm, maxb, lat);
         if (cost < bestc * (1.0 - 1e-9)) { bestc = cost; best = seg; }
     }
     return best;
@@ -782,12 +790,26 @@ void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* t
     const int lim = P.limiter == 0 ? 0 : 1;
     if (dir == 0) {
         const int lines = (P.ny + XW - 1) / XW;
-        const int seg = pick_seg_x(P.nx, lines, num_sms() * NMSDT_X_MINBLOCKS);
+        const int seg = pick_seg_x(P.nx, lines, num_sms(), NMSDT_X_MINBLOCKS, 2.5);
         sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
-        const int seg = pick_seg(P.ny, 1, 128, 4, lines, num_sms() * NMSDT_Y_MINBLOCKS);
+        const int seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 2.6);
         sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg);
+    }
+}
+
+// launch geometry of a fused sweep (sim_sweep_geometry): cells a block marches over, ramp-up cells in front, number of blocks
+void sweep_geometry(const Params& P, int dir, int* seg, int* ramp, long long* nblocks)
+{
+    if (dir == 0) {
+        const int lines = (P.ny + XW - 1) / XW;
+        *seg = pick_seg_x(P.nx, lines, num_sms(), NMSDT_X_MINBLOCKS, 2.5); *ramp = XRAMP;
+        *nblocks = (long long)lines * ((P.nx + *seg - 1) / *seg);
+    } else {
+        const int lines = (P.nx + YT - 1) / YT;
+        *seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 2.6); *ramp = 4;
+        *nblocks = (long long)lines * ((P.ny + *seg - 1) / *seg);
     }
 }
 

@@ -51,6 +51,7 @@ void init_fused_kernels();
 void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* tm_in, double* qout, const double* dtp, Ctl* ctl, int dir, int mode,
                         cudaStream_t s, bool pdl = false);
 void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s);
+void sweep_geometry(const Params& P, int dir, int* seg, int* ramp, long long* nblocks);
 void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s, bool pdl = false);
 double host_tsafe(double tau, double Cpre, double Ta, double theta0);
 int  launch_probe_math(const PowCoef& pw, const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
