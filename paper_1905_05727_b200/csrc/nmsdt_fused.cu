@@ -18,6 +18,7 @@
 //             (128-bit loads/stores).  Neighbour primitives, the right-face state and the face flux cross lanes through
 //             three 33-slot rings of value pairs in shared memory (slot = lane counter mod 33, so lane 31's entry of the previous
 //             chunk is lane 0's left neighbour: no halo recomputation, no copies); 3 __syncwarp per chunk.
+#include <type_traits>
 #include <cuda.h>           // CUtensorMap (type only: the encoder is fetched from the driver at run time, nmsdt_capi.cu)
 #include "nmsdt_host.h"
 #include "nmsdt_fast.cuh"
@@ -315,7 +316,8 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
     int st = pp.st, ph = pp.ph;                   // stage of row jj and the parity of its barrier's current phase
     stage_row(st);
     double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
-    for (int jj = 0; jj < nrows; ++jj) {          // row c = c0 - 2 + jj
+    auto row = [&](auto ramp_tag, int jj) {       // row c = c0 - 2 + jj; RAMP: one of the 4 ramp-up rows (nothing stored or counted)
+        constexpr bool RAMP = decltype(ramp_tag)::value;
         const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
         if (jj + 1 < nrows) {
             __syncwarp(wmask);                    // every lane is done with stage sn (row jj - 2, last read in the previous iteration)
@@ -329,8 +331,6 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
             double dE, q6n;
             prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n, hot);
         }
-        // The body is branch free: during the 4 ramp-up rows it runs on not-yet-valid window / face / flux values
-        // (finite or not, never stored: the store and the wavespeed contribution are predicated on jj >= 4).
         double WL[7], WR[7], lam0c;
         {                                         // centre cell c-1: s_w[0] = W(c-1), s_w[1][0..6] = W(c-1) - W(c-2)
             FCell W0;
@@ -343,7 +343,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
             }
             const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
             lam0c = W0.lam;
-            recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, jj >= 2, hot);      // rows 0, 1: the window is not real yet
+            recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, !RAMP || jj >= 2, hot);      // rows 0, 1: the window is not real yet
             s_w2[0][tid] = make_double2(Wp.r1, Wp.r2); s_w2[1][tid] = make_double2(Wp.un, Wp.ut); s_w2[2][tid] = make_double2(Wp.p, Wp.z1);
             s_w2[3][tid] = make_double2(Wp.lam, Wp.irho); s_w2[4][tid] = make_double2(Wp.rc2, b[0]); s_w2[5][tid] = make_double2(b[1], b[2]);
             s_w2[6][tid] = make_double2(b[3], b[4]); s_w2[7][tid] = make_double2(b[5], b[6]);
@@ -352,7 +352,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         bool oor = false;                         // a face density outside the power tables (only counted once the window is real)
         face_fast<EXACT>(P, s_tab, WL, fl, oor);
         face_fast<EXACT>(P, s_tab, WR, fr, oor);
-        hot |= oor && jj >= 2;
+        hot |= oor && (!RAMP || jj >= 2);
         {
             const double2 r0 = s_r2[0][tid], r1 = s_r2[1][tid], r2 = s_r2[2][tid], r3 = s_r2[3][tid], r4 = s_r2[4][tid];
             pr.r1 = r0.x; pr.r2 = r0.y; pr.un = r1.x; pr.ut = r1.y; pr.p = r2.x; pr.z1 = r2.y; pr.lam = r3.x; pr.rho = r3.y;
@@ -368,7 +368,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
             for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
             o[5] = fma(dtdx * z1n, F[7], o[5]);                           // R8: non-conservative z1 term
             o[5] = clampf(o[5], P.z_min, P.z_max);
-            const bool valid = jj >= 4;
+            constexpr bool valid = !RAMP;
             if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
                 double sm1 = 0.0; int bad1 = 0; bool hot1 = false;
                 trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE, EXACT>(P, s_tab, o, tau, Tsafe, sm1, bad1, hot1);
@@ -393,7 +393,10 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         }
         st = sn;
         ph ^= sn == 0 ? 1 : 0;
-    }
+    };
+    // the 4 ramp-up rows run the same body on a window / face / flux that is not real yet (finite or not: never stored)
+    for (int jj = 0; jj < 4; ++jj) row(std::true_type{}, jj);
+    for (int jj = 4; jj < nrows; ++jj) row(std::false_type{}, jj);
     pp.st = st; pp.ph = ph;                       // (a redo of the segment goes on from here: every staged row has been consumed)
     return hot;
 }
@@ -466,7 +469,11 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + ps), rin + Ac + f * fs);
         cp_async_commit();
     }
-    for (int k = 0; k < niter; ++k) {
+    // EDGE: the first chunk of the segment (ramp-up: lanes 0, 1 update nothing) and the last one (which may end inside the
+    // chunk, at the row end, in the ghost cells).  Every chunk in between updates 64 cells of the segment from 68 cells that all
+    // exist, so its copy of the body carries none of the validity predicates.
+    auto chunk = [&](auto edge_tag, int k) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
         const int b = c0 - XRAMP + 64 * k;           // first cell this iteration would update
         const int A = b + 2 * lane + 2;              // this lane loads cells A, A+1 and reconstructs cells A-1, A
         // In iteration 0 lanes 0, 1 hold the left stencil cells c0-2 .. c0+1: they have no (complete) left neighbours of
@@ -484,15 +491,15 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         cp_async_wait<1>();
         // ---- phase 1: primitives (+ leading source) of the staged pair -----------------------------------------
         {
-            const int Ac = min(max(A, -2), nxe);
+            const int Ac = EDGE ? min(max(A, -2), nxe) : A;
             double qa[7], qb[7];
 #pragma unroll
             for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
             double dE, q6n;
             bool hotb = false;                       // cell Ac + 1 = nx + 2 (odd nx) is row padding, not a cell
-            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qa, (fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
-            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qb, (fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n, hotb);
-            hot |= hotb && Ac <= P.nx;
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qa, (EDGE && fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
+            prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qb, (EDGE && fixed_in && Ac + 1 < 0) ? 0.0 : tau, Tsafe, WB, dE, q6n, hotb);
+            hot |= hotb && (!EDGE || Ac <= P.nx);
             rw[0 * RING + sw] = make_double2(WA.r1, WA.r2); rw[1 * RING + sw] = make_double2(WA.un, WA.ut);
             rw[2 * RING + sw] = make_double2(WA.p, WA.z1);  rw[3 * RING + sw] = make_double2(WA.lam, WB.r1);
             rw[4 * RING + sw] = make_double2(WB.r2, WB.un); rw[5 * RING + sw] = make_double2(WB.ut, WB.p);
@@ -518,8 +525,8 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             // and whose cell is at most the ghost cell nx, the last one a stored face needs.  Cell nx + 1 is reconstructed
             // from cell nx + 2, which does not exist: row padding when nx is odd (its NaN primitives would raise the
             // out-of-table flag on every row end), a clamped reload otherwise.
-            const bool real = k > 0 || lane > 0;
-            const bool cnt1 = real && A - 1 <= P.nx, cnt2 = real && A <= P.nx;
+            const bool real = !EDGE || k > 0 || lane > 0;
+            const bool cnt1 = !EDGE || (real && A - 1 <= P.nx), cnt2 = !EDGE || (real && A <= P.nx);
             bool oor1 = false, oor2 = false;         // a face density outside the power tables
             recon_fast<LIM, EXACT>(P, Wmm, Wm1, WA, khalf, WL, WR, cnt1, hot);
             face_fast<EXACT>(P, s_tab, WL, FL1, oor1);
@@ -553,7 +560,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         // ---- phase 4: update cells A-2 = b + 2 lane and A-1 ---------------------------------------------------
         const int u0 = b + 2 * lane;
         {
-            const bool valid = u0 >= c0 && u0 < c1;
+            const bool valid = !EDGE || (u0 >= c0 && u0 < c1);
             double F0[8];
 #pragma unroll
             for (int f = 0; f < 4; ++f) { const double2 v = rf[f * RING + sr]; F0[2 * f] = v.x; F0[2 * f + 1] = v.y; }
@@ -570,7 +577,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             for (int f = 0; f < 7; ++f) { oa[f] = fma(-dtdx, F1[f] - F0[f], oa[f]); ob[f] = fma(-dtdx, F2[f] - F1[f], ob[f]); }
             oa[5] = clampf(fma(dtdx * za, F1[7] - F0[7], oa[5]), P.z_min, P.z_max);       // R8
             ob[5] = clampf(fma(dtdx * zb, F2[7] - F1[7], ob[5]), P.z_min, P.z_max);
-            const bool two = u0 + 1 < c1;
+            const bool two = !EDGE || u0 + 1 < c1;
             if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
                 double sm1 = 0.0, sm2 = 0.0; int bad1 = 0, bad2 = 0; bool hot1 = false, hot2 = false;
                 trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE, EXACT>(P, s_tab, oa, tau, Tsafe, sm1, bad1, hot1);
@@ -591,6 +598,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         }
         sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
         ps = psn;
+    };
+    for (int k = 0; k < niter; ++k) {
+        if (k == 0 || k == niter - 1) chunk(std::true_type{}, k);
+        else chunk(std::false_type{}, k);
     }
     cp_async_wait<0>();
     return hot;
