@@ -218,10 +218,12 @@ int sim_slab_ipc_close(void* device_base);
 
 /* Select kernel variant (SIM_VARIANT_*) and whether sim_step replays CUDA graphs (default on). */
 int sim_set_variant(sim_t*, int variant, int use_graph);
-/* How sim_step enqueues the fused variant's kernels (5 per step): use_graph = pairs of steps replayed as one CUDA graph
-   (default on), use_pdl = the kernels chained by programmatic dependent launch, a kernel's prologue overlapping its
-   predecessor's tail (default off: measured 3-6 % slower than plain graph edges on the launch-bound configs, equal on
-   the large ones).  They change when kernels start, never what they compute. */
+/* How sim_step enqueues the fused variant's kernels (2 per step: pass 1 and pass 2; ghost cells are taken from the
+   boundary rule as the sweeps load them and the last block of pass 2 ends the step, so there is no halo or control
+   launch): use_graph = pairs of steps replayed as one CUDA graph (default on), use_pdl = the kernels chained by
+   programmatic dependent launch, a kernel's prologue overlapping its predecessor's tail (default off: measured 3-6 %
+   slower than plain graph edges on the launch-bound configs, equal on the large ones).  They change when
+   kernels start, never what they compute. */
 int sim_set_launch_mode(sim_t*, int use_graph, int use_pdl);
 /* Launch geometry of the fused sweep in direction dir (0 = x, 1 = y) on this grid: a block (y: 128 columns, x: 4 rows)
    marches over *seg cells after *ramp recomputed ramp-up cells; *nblocks blocks per launch.  The kernels execute

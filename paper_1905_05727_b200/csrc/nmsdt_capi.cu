@@ -129,7 +129,7 @@ void fill_params(sim* s)
     P.A = e.A; P.B = e.B; P.C = e.C; P.D = e.D; P.rho02 = e.rho02; P.irho02 = 1.0 / e.rho02; P.cv2 = e.cv2; P.Tref2 = e.Tref2;
     P.kA = -e.A / (1.0 - e.C); P.kB = e.B / (1.0 - e.D); P.AC = e.A * e.C; P.BD = e.B * e.D;
     P.z_min = e.z_min; P.z_max = 1.0 - e.z_min;
-    P.C2 = e.C * LOG2E; P.D2 = e.D * LOG2E; P.iG2cv2 = 1.0 / (e.Gamma2 * e.cv2); P.tab = s->tab;
+    P.C2 = e.C * LOG2E; P.D2 = e.D * LOG2E; P.iG2cv2 = 1.0 / (e.Gamma2 * e.cv2); P.tab = s->tab; P.inflow = s->inflow;
     fill_pow_coef(P.pw, e.C, e.D);
     P.g1iG1 = e.gamma1 / (e.gamma1 - 1.0);
     // rho2 e_ref2 - p_ref2/Gamma2 = E1 x^C + E2 x^D - E3 x and rho2 c2^2 - (Gamma2+1) p = R1 x^C + R2 x^D  (Eq. 3-4 in O2)
@@ -258,7 +258,7 @@ void enqueue_step_unfused(sim* s)
     s->host_step++;
 }
 
-// one full step on the fused path: [halo, S(dt/2)+sweep d1] [halo, sweep d2 + S(dt/2) + CFL partial] [ctl]
+// one full step on the fused path: [S(dt/2) + sweep d1] [sweep d2 + S(dt/2) + CFL partial + end of step]
 void enqueue_step_fused(sim* s)
 {
     cudaStream_t st = s->stream;
@@ -266,16 +266,15 @@ void enqueue_step_fused(sim* s)
     const double* dtp = &s->ctl->dt;
     const int d1 = (s->host_step & 1) ? 1 : 0, d2 = 1 - d1;
     const bool pdl = s->use_pdl && !s->profile;      // (event pairs between the kernels would serialise them anyway)
-    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->A, s->inflow, d1, st, pdl); }
+    // (no halo launches: the fused sweeps take ghost cells from the boundary rule as they load them, ghost_src in nmsdt_fused.cu)
     { KTimer t(s, d1 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->A, &s->tmA, s->B, dtp, s->ctl, d1, 1, st, pdl); }
-    { KTimer t(s, SIM_K_HALO); launch_halo(P, s->B, s->inflow, d2, st, pdl); }
-    { KTimer t(s, d2 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->B, &s->tmB, s->A, dtp, s->ctl, d2, 2, st, pdl); }
-    { KTimer t(s, SIM_K_CFL); launch_ctl(P, s->ctl, 1, st, pdl); }
-    s->launches += 5;
+    // (the step is ended -- t, step counter, next dt -- by the last block of the pass-2 sweep to finish: no k_ctl launch)
+    { KTimer t(s, d2 == 0 ? SIM_K_SWEEP_X : SIM_K_SWEEP_Y); launch_sweep_fused(P, s->B, &s->tmB, s->A, dtp, s->ctl, d2, 2, st, pdl, true); }
+    s->launches += 2;
     s->host_step++;
 }
 
-// fused path: CUDA graph of two consecutive steps starting at an even step.  Captured once on a private stream
+// fused path: CUDA graph of two consecutive steps (2 x 2 kernels) starting at an even step.  Captured once on a private stream
 // (nothing executes during capture; every kernel argument is fixed for the lifetime of the handle) and replayed on
 // the caller's stream, which removes the per-launch CPU cost that dominates the small configs (C1, C2).
 bool ensure_graph(sim* s)
@@ -508,7 +507,7 @@ static int step_common(sim_t* s, int n, double dt_fixed)
         if (ensure_graph(s)) {
             for (; n >= 2; n -= 2) {
                 if (cudaGraphLaunch(s->gexec, s->stream) != cudaSuccess) return check_cuda(s, "sim_step (graph)");
-                s->launches += 10; s->host_step += 2;
+                s->launches += 4; s->host_step += 2;
             }
         }
     }

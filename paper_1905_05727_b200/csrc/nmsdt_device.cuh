@@ -32,6 +32,7 @@ struct Params {
     double E1, E2, E3, R1, R2;   // Eq. 3-4 folded into the closure: see face_fast / prim_cell
     PowCoef pw;                  // exponents C, D of Eq. 3-4 and their binomial coefficients (q_pow_tab)
     const double* tab;
+    const double* inflow;        // [7][ny] left boundary column captured by sim_init* (SIM_BC_INFLOW_FIXED)
 };
 
 // device-resident control block: the time step never visits the host inside sim_step
@@ -45,6 +46,8 @@ struct Ctl {
     unsigned long long smax_bits; // max wavespeed of the current state, as ordered bits of a non-negative double
     int bad;
     int redo;                     // fused path: warp segments repeated with the exact rules since sim_init (R13 / R17 / power tables)
+    unsigned int ticket;          // fused path: blocks of the running pass-2 sweep that have finished (the last one ends the step)
+    int pad;
 };
 
 // Programmatic dependent launch (the step's kernels are chained with it, nmsdt_capi.cu): a kernel lets the next one in the

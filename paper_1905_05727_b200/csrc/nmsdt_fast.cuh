@@ -31,29 +31,35 @@ __device__ __noinline__ int nsub_exact(const Params& P, double Tub, double tau)
     return (r >= (double)(P.max_substeps - 1)) ? P.max_substeps : 1 + (int)r;
 }
 
-// Arrhenius factor of Eq. 6 at (l, T): l exp(-Ta/T) for T > 0, else 0 (O5); the rate is -C times this.  One range test
-// on the high word of y = Ta/T covers both guards: y in [0, 690) <=> T > 0 and exp(-y) above ~1e-300 (the rate is taken
-// as 0 beyond that; 690 = 0x40859000_00000000); T <= 0, T = +0 (y = inf) and NaN all fail the unsigned compare.
-__device__ __forceinline__ double arr_factor(const Params& P, const double* __restrict__ tab, double l, double T)
+// Arrhenius factor of Eq. 6 at (l, T) without its guard: l exp(-Ta/T); the rate is -C times this.  `good` reports the guard
+// of O5 (T > 0, else the rate is 0) as one range test on the high word of y = Ta/T: y in [0, 690) <=> T > 0 and exp(-y) above
+// ~1e-300 (the rate is taken as 0 beyond that; 690 = 0x40859000_00000000); T <= 0, T = +0 (y = inf) and NaN all fail the
+// unsigned compare.
+__device__ __forceinline__ double arr_factor(const Params& P, const double* __restrict__ tab, double l, double T, bool& good)
 {
     const double y = P.Ta * q_rcp(T);
-    const bool good = (unsigned)hi_word(y) < 0x40859000u;
-    const double k = l * q_exp2_prod(tab, y, -KC[9]);
-    return good ? k : 0.0;
+    good = (unsigned)hi_word(y) < 0x40859000u;
+    return l * q_exp2_prod(tab, y, -KC[9]);
 }
 
 // one classic RK4 step of d(lambda)/dt = -lambda C exp(-Ta/T2(lambda)), T2 = T0 + beta (lam0 - lambda), from lam over h.
 // The constant -C rides on the step (hC = -h C, stages k_i / (-C)) and T2 = Tb - beta lambda with Tb = T0 + beta lam0:
 // 8 FP64 instructions fewer than the literal form, same values up to rounding.
+// O5 tests T > 0 at every stage; one test decides all four.  If the first stage fails it, k1 = 0, the second stage sits at the
+// same lambda and temperature and fails too, and so on: lambda is returned unchanged.  If it passes, the stage values of
+// lambda never exceed lam (h C k >= 0 is subtracted), so with beta > 0 every later stage is at least as hot and passes.  (The
+// trace liquid inside a collapsing cavity, compressed along with the air, does sit below its reference curve: T2 < 0 there.)
 __device__ __forceinline__ double rk4_step(const Params& P, const double* __restrict__ tab, double Tb, double beta, double lam, double h)
 {
     const double hC = -h * P.Cpre, nb = -beta;
     double l, k1, k2, k3, k4;
-    l = lam;                       k1 = arr_factor(P, tab, l, fma(nb, l, Tb));
-    l = fma(0.5 * hC, k1, lam);    k2 = arr_factor(P, tab, l, fma(nb, l, Tb));
-    l = fma(0.5 * hC, k2, lam);    k3 = arr_factor(P, tab, l, fma(nb, l, Tb));
-    l = fma(hC, k3, lam);          k4 = arr_factor(P, tab, l, fma(nb, l, Tb));
-    return fma(hC * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
+    bool good, g;
+    l = lam;                       k1 = arr_factor(P, tab, l, fma(nb, l, Tb), good);
+    l = fma(0.5 * hC, k1, lam);    k2 = arr_factor(P, tab, l, fma(nb, l, Tb), g);
+    l = fma(0.5 * hC, k2, lam);    k3 = arr_factor(P, tab, l, fma(nb, l, Tb), g);
+    l = fma(hC, k3, lam);          k4 = arr_factor(P, tab, l, fma(nb, l, Tb), g);
+    const double r = fma(hC * (1.0 / 6.0), (k1 + k4) + 2.0 * (k2 + k3), lam);
+    return good ? r : lam;
 }
 
 // R13 sub-stepped integration (only reached by cells hotter than the safe bound)

@@ -206,6 +206,67 @@ __device__ __forceinline__ void lead_fix(const Params& P, double q[7], double la
     q[6] = q6n;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// end of a step: t, step counter, next dt from the max wavespeed (a7, R11) and the temperature bound below which the R13
+// rule certainly gives n_sub = 1 for tau = dt/2.  Run by one thread: of k_ctl, or of the last block of the step's pass-2
+// sweep to finish (step_end_by_last_block), which saves the launch.
+// ---------------------------------------------------------------------------------------------------------------
+__host__ __device__ inline double tsafe_for(double tau, double Cpre, double Ta, double theta0)
+{
+    // n_sub = 1 + floor(tau C g(Ta/T) / theta0), g(y) = 1/(1 + y + y^2/2 + y^3/6) decreasing in y.
+    // Return T* such that T < T* guarantees tau C g < theta0 (1 - 1e-6); +inf when that holds for every T.
+    const double target = theta0 * (1.0 - 1e-6) / (tau * Cpre);       // need g(y) < target
+    if (!(tau > 0.0) || target >= 1.0) return 1e300;
+    // y* = positive root of h(y) = 1 + y + y^2/2 + y^3/6 - 1/target (h' > 0, h'' > 0 for y > 0).  Newton from
+    // y0 = cbrt(6/target), where h(y0) = 1 + y0 + y0^2/2 > 0: the iterates fall monotonically onto the root from the right,
+    // so every one of them is a safe bound (y_n >= y*  =>  Ta/y_n <= Ta/y*).  A dozen divisions instead of the 64
+    // bisections of round 1.
+    const double r = 1.0 / target;
+    double y = cbrt(6.0 * r);
+    for (int it = 0; it < 12; ++it) {
+        const double h = 1.0 + y * (1.0 + y * (0.5 + y * (1.0 / 6.0))) - r;
+        const double dh = 1.0 + y * (1.0 + 0.5 * y);
+        const double yn = y - h / dh;
+        if (!(yn < y)) break;                                         // converged (or rounding would step back over the root)
+        y = yn;
+    }
+    return Ta / (y * (1.0 + 1e-12));                                  // T < Ta/y  =>  Ta/T > y >= y*  =>  g < target
+}
+
+__device__ __forceinline__ void ctl_update(const Params& P, Ctl* ctl, int advance)
+{
+    if (advance) { ctl->t += ctl->dt; ctl->dt_last = ctl->dt; ctl->step += 1; }
+    const double smax = __longlong_as_double((long long)atomicMax(&ctl->smax_bits, 0ull));    // (read at the point of coherence)
+    const double dt = ctl->dt_fixed > 0.0 ? ctl->dt_fixed : P.cfl * P.hmin / smax;
+    ctl->dt = dt;
+    ctl->tsafe = P.reactive ? tsafe_for(0.5 * dt, P.Cpre, P.Ta, P.theta0) : 1e300;
+    ctl->smax_bits = 0ull;
+}
+
+__global__ void k_ctl(const __grid_constant__ Params P, Ctl* ctl, int advance)
+{
+    pdl_launch_dependents();
+    pdl_wait();
+    ctl_update(P, ctl, advance);
+}
+
+// Last instruction block of a pass-2 sweep kernel: every block takes a ticket once its warps have added their wavespeed
+// maxima; the block that takes the last one has seen all of them (fence, then ticket) and ends the step.  Every block has
+// read dt long before (at its start), so overwriting ctl->dt here is safe; the next kernel starts after this one has ended.
+__device__ __forceinline__ void step_end_by_last_block(const Params& P, Ctl* ctl)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned total = gridDim.x * gridDim.y;
+        if (atomicAdd(&ctl->ticket, 1u) == total - 1u) {
+            __threadfence();
+            ctl_update(P, ctl, 1);
+            ctl->ticket = 0u;
+        }
+    }
+}
+
 #ifndef NMSDT_Y_MINBLOCKS
 #define NMSDT_Y_MINBLOCKS 4
 #endif
@@ -220,6 +281,33 @@ constexpr int PRING = 66;                   // staged input pairs: chunk k (32 s
 constexpr int XS_DOUBLES = XW * (RING_DOUBLES + 7 * PRING * 2);    // dynamic part (the math tables are static)
 
 } // namespace
+
+// ---------------------------------------------------------------------------------------------------------------
+// Boundary rules folded into the sweeps (a2; P:129 transmissive inflow, P:135 periodic top / bottom; R12): a ghost cell is
+// never read from memory, its value is taken from the cell the rule names when the sweep loads it -- in the copies of the
+// loop bodies that handle segment edges only, so the marching loops proper do not pay for it, and a step needs no halo
+// launch.  Cell index c of a line of n cells, c in [-2, -1] or [n, n+1]:
+//   transmissive (0): nearest interior cell;  periodic (1): c -+ n;  reflective (2): mirror image, normal momentum negated;
+//   fixed inflow (3, x-lo only): the column captured by sim_init;  external (4, x only): the stored ghost column (a
+//   neighbour slab's cells, written by the slab exchange).
+// ghost_src returns the interior index the value comes from (and whether the normal momentum changes sign), or -1 when the
+// stored / staged value is to be used as it is (interior cell, external side, fixed inflow -- handled by the caller).
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int ghost_src(int c, int n, int bc_lo, int bc_hi, bool& flip)
+{
+    flip = false;
+    if (c < 0) {
+        if (bc_lo == 1) return ((c % n) + n) % n;
+        if (bc_lo == 2) { flip = true; return min(-1 - c, n - 1); }
+        return bc_lo == 0 ? 0 : -1;
+    }
+    if (c >= n) {
+        if (bc_hi == 1) return (c - n) % n;
+        if (bc_hi == 2) { flip = true; return max(2 * n - 1 - c, 0); }
+        return bc_hi == 0 ? n - 1 : -1;
+    }
+    return -1;
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // input staging: cp.async (x-sweep), bulk tensor copies + mbarriers (y-sweep)
@@ -299,35 +387,39 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
     const long long fs = P.fstride, pitch = P.pitch;
     double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
     const int nrows = c1 - c0 + 4;
-    // one lane per warp stages a row: the {32, 1, 7} box at (first column of the warp, row, plane 0) of the input plane set
+    // one lane per warp stages a row: the {32, 1, 7} box at (first column of the warp, row, plane 0) of the input plane set.
+    // `r` is the row of the grid, -2 .. ny + 1; a ghost row (only ever staged and read by the EDGE copy of the body) is taken
+    // from the interior row the boundary rule names (ghost_src), its normal momentum negated on read where the wall reflects.
     const int tx = NGX + col - lane;
-    int ty = c0 - 2 + NGY;
-    auto stage_row = [&](int sg) {
+    auto stage_row = [&](int sg, int r, bool edge) {
         if (lane == 0) {
+            bool flip;
+            const int src = edge ? ghost_src(r, P.ny, P.bc_ylo, P.bc_yhi, flip) : -1;
             mbar_expect_tx(&bars[sg], 7 * 32 * (int)sizeof(double));
-            tma_load_3d(&s_st[sg][0][0], tm, tx, ty, 0, &bars[sg]);
+            tma_load_3d(&s_st[sg][0][0], tm, tx, (src >= 0 ? src : r) + NGY, 0, &bars[sg]);
         }
-        ++ty;
     };
     auto read_row = [&](int sg, double q[7]) {            // sweep field order: q0, q1, q3 (normal), q2 (tangential), q4, q5, q6
         q[0] = s_st[sg][0][lane]; q[1] = s_st[sg][1][lane]; q[2] = s_st[sg][3][lane]; q[3] = s_st[sg][2][lane];
         q[4] = s_st[sg][4][lane]; q[5] = s_st[sg][5][lane]; q[6] = s_st[sg][6][lane];
     };
+    auto reflected = [&](int r) { return (r < 0 && P.bc_ylo == 2) || (r >= P.ny && P.bc_yhi == 2); };
     int st = pp.st, ph = pp.ph;                   // stage of row jj and the parity of its barrier's current phase
-    stage_row(st);
+    stage_row(st, c0 - 2, true);
     double acc[7] = {0, 0, 0, 0, 0, 0, 0}, z1n = 0.0;
-    auto row = [&](auto ramp_tag, int jj) {       // row c = c0 - 2 + jj; RAMP: one of the 4 ramp-up rows (nothing stored or counted)
-        constexpr bool RAMP = decltype(ramp_tag)::value;
+    auto row = [&](auto edge_tag, int jj) {       // row c = c0 - 2 + jj; EDGE: a ramp-up row or one of the last 3 (see below)
+        constexpr bool EDGE = decltype(edge_tag)::value;
         const int sn = st == YST - 1 ? 0 : st + 1, sp = st == 0 ? YST - 1 : st - 1;
-        if (jj + 1 < nrows) {
+        if (!EDGE || jj + 1 < nrows) {
             __syncwarp(wmask);                    // every lane is done with stage sn (row jj - 2, last read in the previous iteration)
-            stage_row(sn);
+            stage_row(sn, c0 - 1 + jj, EDGE);
         }
         mbar_wait(&bars[st], ph);
         FCell Wp;
         {
             double q[7];
             read_row(st, q);
+            if (EDGE && reflected(c0 - 2 + jj)) q[2] = -q[2];
             double dE, q6n;
             prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, q, tau, Tsafe, Wp, dE, q6n, hot);
         }
@@ -343,7 +435,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
             }
             const double b[7] = {Wp.r1 - W0.r1, Wp.r2 - W0.r2, Wp.un - W0.un, Wp.ut - W0.ut, Wp.p - W0.p, Wp.z1 - W0.z1, Wp.lam - W0.lam};
             lam0c = W0.lam;
-            recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, !RAMP || jj >= 2, hot);      // rows 0, 1: the window is not real yet
+            recon_core<LIM, EXACT>(P, W0, a, b, khalf, WL, WR, !EDGE || jj >= 2, hot);      // rows 0, 1: the window is not real yet
             s_w2[0][tid] = make_double2(Wp.r1, Wp.r2); s_w2[1][tid] = make_double2(Wp.un, Wp.ut); s_w2[2][tid] = make_double2(Wp.p, Wp.z1);
             s_w2[3][tid] = make_double2(Wp.lam, Wp.irho); s_w2[4][tid] = make_double2(Wp.rc2, b[0]); s_w2[5][tid] = make_double2(b[1], b[2]);
             s_w2[6][tid] = make_double2(b[3], b[4]); s_w2[7][tid] = make_double2(b[5], b[6]);
@@ -352,7 +444,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         bool oor = false;                         // a face density outside the power tables (only counted once the window is real)
         face_fast<EXACT>(P, s_tab, WL, fl, oor);
         face_fast<EXACT>(P, s_tab, WR, fr, oor);
-        hot |= oor && (!RAMP || jj >= 2);
+        hot |= oor && (!EDGE || jj >= 2);
         {
             const double2 r0 = s_r2[0][tid], r1 = s_r2[1][tid], r2 = s_r2[2][tid], r3 = s_r2[3][tid], r4 = s_r2[4][tid];
             pr.r1 = r0.x; pr.r2 = r0.y; pr.un = r1.x; pr.ut = r1.y; pr.p = r2.x; pr.z1 = r2.y; pr.lam = r3.x; pr.rho = r3.y;
@@ -368,7 +460,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
             for (int k = 0; k < 7; ++k) o[k] = fma(-dtdx, F[k], acc[k]);
             o[5] = fma(dtdx * z1n, F[7], o[5]);                           // R8: non-conservative z1 term
             o[5] = clampf(o[5], P.z_min, P.z_max);
-            constexpr bool valid = !RAMP;
+            const bool valid = !EDGE || jj >= 4;             // (the ramp-up rows finish nothing)
             if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
                 double sm1 = 0.0; int bad1 = 0; bool hot1 = false;
                 trail_cell<MODE == MODE_TRAIL ? SRC : SRC_NONE, EXACT>(P, s_tab, o, tau, Tsafe, sm1, bad1, hot1);
@@ -384,7 +476,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         }
         {                                         // start cell c-1 with its lower-face flux
             double o[7];
-            read_row(sp, o);
+            read_row(sp, o);                      // (row jj - 1 is a cell of the segment whenever what starts here is kept: no ghost rule)
             if (MODE == MODE_LEAD) lead_fix(P, o, lam0c);
             z1n = o[5];
 #pragma unroll
@@ -394,16 +486,20 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         st = sn;
         ph ^= sn == 0 ? 1 : 0;
     };
-    // the 4 ramp-up rows run the same body on a window / face / flux that is not real yet (finite or not: never stored)
+    // EDGE copy of the body: the 4 ramp-up rows, which run on a window / face / flux that is not real yet (finite or
+    // not: nothing is stored or counted), and the last 3 rows, which stage and read the rows beyond the segment end -- ghost rows
+    // when the segment ends at the grid's.  The rows in between touch cells of the grid only.
+    const int jmid = nrows - 3 > 4 ? nrows - 3 : 4;
     for (int jj = 0; jj < 4; ++jj) row(std::true_type{}, jj);
-    for (int jj = 4; jj < nrows; ++jj) row(std::false_type{}, jj);
+    for (int jj = 4; jj < jmid; ++jj) row(std::false_type{}, jj);
+    for (int jj = jmid; jj < nrows; ++jj) row(std::true_type{}, jj);
     pp.st = st; pp.ph = ph;                       // (a redo of the segment goes on from here: every staged row has been consumed)
     return hot;
 }
 
 template <int MODE, int LIM>
 __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const __grid_constant__ CUtensorMap tm,
-                                                                  double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg)
+                                                                  double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg, int end_step)
 {
     extern __shared__ __align__(16) double s_dyn_raw[];
     // the staged rows are bulk-copy destinations and must be 128-byte aligned: the dynamic part follows the static arrays
@@ -430,7 +526,10 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
             y_segment<MODE, true, LIM>(P, qout, dtp, seg, col, s_tab, s_dyn, smax, bad, &tm, bars, wmask, pp);
         }
     }
-    if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
+    if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
+        reduce_smax(smax, bad, ctl);
+        if (end_step) step_end_by_last_block(P, ctl);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -469,8 +568,8 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + ps), rin + Ac + f * fs);
         cp_async_commit();
     }
-    // EDGE: the first chunk of the segment (ramp-up: lanes 0, 1 update nothing) and the last one (which may end inside the
-    // chunk, at the row end, in the ghost cells).  Every chunk in between updates 64 cells of the segment from 68 cells that all
+    // EDGE: the first chunk of the segment (ramp-up: lanes 0, 1 update nothing; ghost cells of the row start) and the last one or
+    // two (which end inside the chunk, at the row end, in the ghost cells: those get their values from the boundary rule).  Every chunk in between updates 64 cells of the segment from 68 cells that all
     // exist, so its copy of the body carries none of the validity predicates.
     auto chunk = [&](auto edge_tag, int k) {
         constexpr bool EDGE = decltype(edge_tag)::value;
@@ -495,6 +594,24 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             double qa[7], qb[7];
 #pragma unroll
             for (int f = 0; f < 7; ++f) { const double2 v = stg[f * PRING + ps]; qa[f] = v.x; qb[f] = v.y; }
+            if (EDGE && (Ac < 0 || Ac + 1 >= P.nx)) {              // a ghost cell in the pair: apply the boundary rule (see ghost_src)
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int c = Ac + h;
+                    double* q = h == 0 ? qa : qb;
+                    if (c > P.nx + 1) continue;                   // row padding (odd nx): not a cell, never used
+                    bool flip;
+                    const int src = ghost_src(c, P.nx, P.bc_xlo, P.bc_xhi, flip);
+                    if (src >= 0) {
+#pragma unroll
+                        for (int f = 0; f < 7; ++f) q[f] = rin[src + f * fs];
+                        if (flip) q[2] = -q[2];
+                    } else if (c < 0 && P.bc_xlo == 3) {
+#pragma unroll
+                        for (int f = 0; f < 7; ++f) q[f] = P.inflow[f * P.ny + row];
+                    }
+                }
+            }
             double dE, q6n;
             bool hotb = false;                       // cell Ac + 1 = nx + 2 (odd nx) is row padding, not a cell
             prim_cell<MODE == MODE_LEAD ? SRC : SRC_NONE, EXACT>(P, s_tab, qa, (EDGE && fixed_in && Ac < 0) ? 0.0 : tau, Tsafe, WA, dE, q6n, hot);
@@ -600,7 +717,8 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         ps = psn;
     };
     for (int k = 0; k < niter; ++k) {
-        if (k == 0 || k == niter - 1) chunk(std::true_type{}, k);
+        // a middle chunk loads cells b + 2 .. b + 65, all of them cells of the row below the segment end
+        if (k == 0 || c0 - XRAMP + 64 * k + 65 >= c1) chunk(std::true_type{}, k);
         else chunk(std::false_type{}, k);
     }
     cp_async_wait<0>();
@@ -609,7 +727,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
 
 template <int MODE, int LIM>
 __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
-                                                    const double* __restrict__ dtp, Ctl* ctl, int seg)
+                                                    const double* __restrict__ dtp, Ctl* ctl, int seg, int end_step)
 {
     extern __shared__ __align__(16) double s_dyn[];
     __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
@@ -628,7 +746,10 @@ __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __g
             x_segment<MODE, true, LIM>(P, qin, qout, dtp, seg, row, s_tab, s_dyn, smax, bad);
         }
     }
-    if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) reduce_smax(smax, bad, ctl);
+    if (MODE == MODE_TRAIL || MODE == MODE_TRAIL_INERT) {
+        reduce_smax(smax, bad, ctl);
+        if (end_step) step_end_by_last_block(P, ctl);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -650,44 +771,6 @@ __global__ void __launch_bounds__(128) k_source_fast(const __grid_constant__ Par
     prim_cell<SRC_EXACT>(P, s_tab, c, dtp[0], dtp[1], W, dE, q6n, hot);
     q[4 * P.fstride + id] = c[4] + dE;
     q[6 * P.fstride + id] = q6n;
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// one-thread control kernel: finish the step (t, step counter), next dt from the max wavespeed (a7, R11) and the
-// temperature bound below which the R13 rule certainly gives n_sub = 1 for tau = dt/2
-// ---------------------------------------------------------------------------------------------------------------
-__host__ __device__ inline double tsafe_for(double tau, double Cpre, double Ta, double theta0)
-{
-    // n_sub = 1 + floor(tau C g(Ta/T) / theta0), g(y) = 1/(1 + y + y^2/2 + y^3/6) decreasing in y.
-    // Return T* such that T < T* guarantees tau C g < theta0 (1 - 1e-6); +inf when that holds for every T.
-    const double target = theta0 * (1.0 - 1e-6) / (tau * Cpre);       // need g(y) < target
-    if (!(tau > 0.0) || target >= 1.0) return 1e300;
-    // y* = positive root of h(y) = 1 + y + y^2/2 + y^3/6 - 1/target (h' > 0, h'' > 0 for y > 0).  Newton from
-    // y0 = cbrt(6/target), where h(y0) = 1 + y0 + y0^2/2 > 0: the iterates fall monotonically onto the root from the right,
-    // so every one of them is a safe bound (y_n >= y*  =>  Ta/y_n <= Ta/y*).  This runs in the one-thread k_ctl of every
-    // step: a dozen divisions instead of the 64 bisections it replaced (12.8 -> ~2 us per step).
-    const double r = 1.0 / target;
-    double y = cbrt(6.0 * r);
-    for (int it = 0; it < 12; ++it) {
-        const double h = 1.0 + y * (1.0 + y * (0.5 + y * (1.0 / 6.0))) - r;
-        const double dh = 1.0 + y * (1.0 + 0.5 * y);
-        const double yn = y - h / dh;
-        if (!(yn < y)) break;                                         // converged (or rounding would step back over the root)
-        y = yn;
-    }
-    return Ta / (y * (1.0 + 1e-12));                                  // T < Ta/y  =>  Ta/T > y >= y*  =>  g < target
-}
-
-__global__ void k_ctl(const __grid_constant__ Params P, Ctl* ctl, int advance)
-{
-    pdl_launch_dependents();
-    pdl_wait();
-    if (advance) { ctl->t += ctl->dt; ctl->dt_last = ctl->dt; ctl->step += 1; }
-    const double smax = __longlong_as_double((long long)ctl->smax_bits);
-    const double dt = ctl->dt_fixed > 0.0 ? ctl->dt_fixed : P.cfl * P.hmin / smax;
-    ctl->dt = dt;
-    ctl->tsafe = P.reactive ? tsafe_for(0.5 * dt, P.Cpre, P.Ta, P.theta0) : 1e300;
-    ctl->smax_bits = 0ull;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -751,28 +834,28 @@ static int num_sms()
 
 template <int MODE, int LIM>
 static void x_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, bool pdl, const Params& P, const double* qin, double* qout, const double* dtp,
-                     Ctl* ctl, int seg)
+                     Ctl* ctl, int seg, int end_step)
 {
     if (attr_only) cudaFuncSetAttribute(k_xsweep<MODE, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    else launch_k(k_xsweep<MODE, LIM>, grid, dim3(32 * XW), sm, s, pdl, P, qin, qout, dtp, ctl, seg);
+    else launch_k(k_xsweep<MODE, LIM>, grid, dim3(32 * XW), sm, s, pdl, P, qin, qout, dtp, ctl, seg, end_step);
 }
 template <int MODE, int LIM>
 static void y_launch(bool attr_only, dim3 grid, size_t sm, cudaStream_t s, bool pdl, const Params& P, const CUtensorMap* tm, double* qout, const double* dtp,
-                     Ctl* ctl, int seg)
+                     Ctl* ctl, int seg, int end_step)
 {
     if (attr_only) cudaFuncSetAttribute(k_ysweep<MODE, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    else launch_k(k_ysweep<MODE, LIM>, grid, dim3(YT), sm, s, pdl, P, *tm, qout, dtp, ctl, seg);
+    else launch_k(k_ysweep<MODE, LIM>, grid, dim3(YT), sm, s, pdl, P, *tm, qout, dtp, ctl, seg, end_step);
 }
 
 // dispatch on (direction, pass kind, limiter); attr_only = opt in to the dynamic shared memory instead of launching
 static void sweep_dispatch(bool attr_only, int dir, int mode, int lim, dim3 grid, cudaStream_t s, bool pdl, const Params& P, const double* qin,
-                           const CUtensorMap* tm, double* qout, const double* dtp, Ctl* ctl, int seg)
+                           const CUtensorMap* tm, double* qout, const double* dtp, Ctl* ctl, int seg, int end_step)
 {
     const size_t sm = (dir == 0 ? XS_DOUBLES : YS_DOUBLES) * sizeof(double);
 #define NMSDT_CASE(D, M, L)                                                                                          \
     if (dir == D && mode == M && lim == L) {                                                                        \
-        if (D == 0) x_launch<M, L>(attr_only, grid, sm, s, pdl, P, qin, qout, dtp, ctl, seg);                     \
-        else        y_launch<M, L>(attr_only, grid, sm, s, pdl, P, tm, qout, dtp, ctl, seg);                      \
+        if (D == 0) x_launch<M, L>(attr_only, grid, sm, s, pdl, P, qin, qout, dtp, ctl, seg, end_step);                   \
+        else        y_launch<M, L>(attr_only, grid, sm, s, pdl, P, tm, qout, dtp, ctl, seg, end_step);                   \
         return;                                                                                                     \
     }
     NMSDT_CASE(0, MODE_PLAIN, 0) NMSDT_CASE(0, MODE_LEAD, 0) NMSDT_CASE(0, MODE_TRAIL, 0) NMSDT_CASE(0, MODE_TRAIL_INERT, 0)
@@ -788,25 +871,25 @@ void init_fused_kernels()
     Params P{};
     for (int dir = 0; dir < 2; ++dir)
         for (int mode = 0; mode < 4; ++mode)
-            for (int lim = 0; lim < 2; ++lim) sweep_dispatch(true, dir, mode, lim, dim3(1), nullptr, false, P, nullptr, nullptr, nullptr, nullptr, nullptr, 0);
+            for (int lim = 0; lim < 2; ++lim) sweep_dispatch(true, dir, mode, lim, dim3(1), nullptr, false, P, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0);
 }
 
 // mode 0 plain, 1 leading source on load, 2 trailing source + max-wavespeed partial.  An inert run (P.reactive = 0) has
 // no source step: its pass 1 is the plain sweep and its pass 2 the sweep + wavespeed.  The limiter (R5) is a template
 // parameter so that the marching loop stays one basic block.
 void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* tm_in, double* qout, const double* dtp, Ctl* ctl, int dir, int mode, cudaStream_t s,
-                        bool pdl)
+                        bool pdl, bool end_step)
 {
     if (!P.reactive) mode = mode == MODE_LEAD ? MODE_PLAIN : (mode == MODE_TRAIL ? MODE_TRAIL_INERT : mode);
     const int lim = P.limiter == 0 ? 0 : 1;
     if (dir == 0) {
         const int lines = (P.ny + XW - 1) / XW;
         const int seg = pick_seg_x(P.nx, lines, num_sms(), NMSDT_X_MINBLOCKS, 2.5);
-        sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg);
+        sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg, end_step && mode >= MODE_TRAIL ? 1 : 0);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
         const int seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 2.6);
-        sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg);
+        sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg, end_step && mode >= MODE_TRAIL ? 1 : 0);
     }
 }
 

@@ -47,9 +47,10 @@ int  launch_probe_issue(cudaStream_t s, double ms[4]);
 // fused production path (nmsdt_fused.cu). dtp -> {dt (or tau for the source kernel), tsafe}; mode 0 plain, 1 leading
 // source on load, 2 trailing source + max-wavespeed partial
 void init_fused_kernels();
+// end_step (pass 2 only): the last block to finish also ends the step (t, step counter, next dt: what k_ctl does otherwise)
 // tm_in: tensor map of the plane set qin (dims {pitch, rows, 7}, box {32, 1, 7}; make_plane_tensor_map in nmsdt_capi.cu)
 void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* tm_in, double* qout, const double* dtp, Ctl* ctl, int dir, int mode,
-                        cudaStream_t s, bool pdl = false);
+                        cudaStream_t s, bool pdl = false, bool end_step = false);
 void launch_source_fast(const Params& P, double* q, const double* dtp, cudaStream_t s);
 void sweep_geometry(const Params& P, int dir, int* seg, int* ramp, long long* nblocks);
 void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s, bool pdl = false);

@@ -524,3 +524,23 @@ def test_full_size_sampled_parity(O, B, name):
     # global invariants that hold at any size: phase masses change only through the x boundaries (inflow)
     assert d1["mass2"] > d0["mass2"] and d1["bad_state"] == 0
     assert abs(d1["momy"]) < 1e-9 * abs(d1["momx"]) or name != "C3"
+
+
+# ------------------------------------------------------------------------------------------------ launch geometry
+@pytest.mark.parametrize("name,kw", [("C1", {}), ("C2", {}), ("C3", {}), ("C4", {}), ("C5", {}), ("C4", dict(nx=83, ny=37))])
+def test_sweep_geometry_covers_the_grid(B, name, kw):
+    """sim_sweep_geometry: every cell belongs to exactly one segment; grids that fill the GPU get long segments (little ramp-up
+    redundancy), grids that cannot are cut short (latency of the march is what counts there)"""
+    cfg = inputs.config(name, **kw)
+    g = cfg["grid"]
+    s = B.Sim(g, cfg["eos"], cfg["kin"])
+    for d, (n, lines) in enumerate(((g["nx"], (g["ny"] + 3) // 4), (g["ny"], (g["nx"] + 127) // 128))):
+        seg, ramp, nb = s.sweep_geometry(d)
+        assert seg >= 1 and ramp == 4 and nb == lines * ((n + seg - 1) // seg)
+        if d == 0:
+            assert (seg + ramp) % 64 == 0 and seg % 2 == 0                  # whole 64-cell chunks, even starts (pair loads)
+        if name == "C5" and not kw:
+            assert (seg + ramp) / seg < 1.02 and nb > 8 * 148
+        if name in ("C1",) and not kw:
+            assert nb <= 148 * 4 and seg <= (60 if d == 0 else 4)
+    s.close()
