@@ -225,7 +225,7 @@ int sim_set_variant(sim_t*, int variant, int use_graph);
    slower than plain graph edges on the launch-bound configs, equal on the large ones).  They change when
    kernels start, never what they compute. */
 int sim_set_launch_mode(sim_t*, int use_graph, int use_pdl);
-/* Launch geometry of the fused sweep in direction dir (0 = x, 1 = y) on this grid: a block (y: 128 columns, x: 4 rows)
+/* Launch geometry of the fused sweep in direction dir (0 = x, 1 = y) on this grid: a block (y: 256 columns, x: 4 rows)
    marches over *seg cells after *ramp recomputed ramp-up cells; *nblocks blocks per launch.  The kernels execute
    (seg + ramp)/seg times the algorithmic work: the roofline block of bench.py divides that out. */
 int sim_sweep_geometry(const sim_t*, int dir, int* seg, int* ramp, long long* nblocks);

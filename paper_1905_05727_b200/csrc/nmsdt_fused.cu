@@ -31,7 +31,10 @@ namespace {
 // TRAIL_INERT = sweep + wavespeed (inert runs: pass 1 is PLAIN, pass 2 is TRAIL_INERT)
 enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2, MODE_TRAIL_INERT = 3 };
 
-struct FFace { double r1, r2, un, ut, p, z1, lam, rho, rhoE, c; };
+// A face state: the reconstructed primitives, the mixture density and sound speed -- what both sides of a face need for the wave
+// speeds -- and (x^C, x^D) of its liquid density.  The total energy is NOT formed here: only the side the HLLC fan selects needs
+// it, so hllc_fast forms it after the selection from (x^C, x^D) (11 FP64 instructions per face state moved to 12 per face).
+struct FFace { double r1, r2, un, ut, p, z1, lam, rho, c, xC, xD; };
 
 template <bool EX>
 __device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f, bool& oor)
@@ -43,11 +46,8 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     const double x = W[1] * P.irho02;
     double xC, xD;
     eos_pow<EX>(P, tab, x, xC, xD, oor);
-    // Eq. 3-4 enter the closure only through two fixed combinations of x^C, x^D, x (O2):
-    //   (p - p_ref2)/Gamma2 + rho2 e_ref2 = p/Gamma2 + E1 x^C + E2 x^D - E3 x,   rho2 c2^2 = (Gamma2+1) p + R1 x^C + R2 x^D
-    const double brk = fma(p, P.iG2, fma(P.E1, xC, fma(P.E2, xD, -P.E3 * x)));
-    const double kin = 0.5 * rho * fma(W[2], W[2], W[3] * W[3]);
-    f.rhoE = fma(z1 * P.iG1, p, fma(z2, brk, kin));
+    f.xC = xC; f.xD = xD;
+    // Eq. 3-4 enter the sound speed through rho2 c2^2 = (Gamma2+1) p + R1 x^C + R2 x^D (O2)
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double r2c22 = fma(P.R1, xC, fma(P.R2, xD, P.G2p1 * p));
     const double rc2 = fma(z1 * P.g1iG1, p, z2 * P.iG2 * r2c22);
@@ -124,7 +124,7 @@ __device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, con
 }
 
 // O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
-__device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double F[8])
+__device__ __forceinline__ void hllc_fast(const Params& P, const FFace& L, const FFace& R, double F[8])
 {
     const double SL = dmin_(L.un - L.c, R.un - R.c);                  // R9: Davis
     const double SR = dmax_(L.un + L.c, R.un + R.c);
@@ -138,7 +138,12 @@ __device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double
     const bool star = sl_neg && sr_pos;
     const double r1 = useL ? L.r1 : R.r1, r2 = useL ? L.r2 : R.r2, un = useL ? L.un : R.un, ut = useL ? L.ut : R.ut;
     const double p = useL ? L.p : R.p, z1 = useL ? L.z1 : R.z1, lam = useL ? L.lam : R.lam;
-    const double rho = useL ? L.rho : R.rho, rhoE = useL ? L.rhoE : R.rhoE, SK = useL ? SL : SR;
+    const double rho = useL ? L.rho : R.rho, xC = useL ? L.xC : R.xC, xD = useL ? L.xD : R.xD, SK = useL ? SL : SR;
+    // total energy of the selected side (O4.3): Eq. 3-4 enter through (p - p_ref2)/Gamma2 + rho2 e_ref2 = p/Gamma2 + E1 x^C + E2 x^D - E3 x
+    const double z2 = 1.0 - z1;
+    const double brk = fma(p, P.iG2, fma(P.E1, xC, fma(P.E2, xD, -P.E3 * (r2 * P.irho02))));
+    const double kin = 0.5 * rho * fma(un, un, ut * ut);
+    const double rhoE = fma(z1 * P.iG1, p, fma(z2, brk, kin));
     // chi = (SK-un)/(SK-S*) and p/(SK-un) from one reciprocal; outside the fan SKs = 0 and the star terms vanish
     const double a = SK - un, b = SK - Sstar;
     const double rab = star ? q_rcp(a * b) : 0.0;
@@ -148,7 +153,7 @@ __device__ __forceinline__ void hllc_fast(const FFace& L, const FFace& R, double
     // U*_k = chi U_k for the advected components, so F_k = U_k un + SK (chi - 1) U_k = U_k u_face with the
     // HLLC-consistent face velocity u_face = un + SK (chi - 1) (R8)
     const double uf = fma(SKs, chi - 1.0, un);
-    const double U0 = z1 * r1, U1 = (1.0 - z1) * r2;
+    const double U0 = z1 * r1, U1 = z2 * r2;
     F[0] = U0 * uf;
     F[1] = U1 * uf;
     F[2] = fma(rho * un, un, p) + SKs * rho * fma(chi, Sstar, -un);
@@ -268,7 +273,7 @@ __device__ __forceinline__ void step_end_by_last_block(const Params& P, Ctl* ctl
 }
 
 #ifndef NMSDT_Y_MINBLOCKS
-#define NMSDT_Y_MINBLOCKS 4
+#define NMSDT_Y_MINBLOCKS 2
 #endif
 #ifndef NMSDT_X_MINBLOCKS
 #define NMSDT_X_MINBLOCKS 3
@@ -276,7 +281,7 @@ __device__ __forceinline__ void step_end_by_last_block(const Params& P, Ctl* ctl
 constexpr int XW = 4;                       // warps per block in k_xsweep
 constexpr int RING = 33;
 constexpr int XRAMP = 4;                    // cells left of a segment that k_xsweep recomputes (stencil radius 2, two passes of neighbours)
-constexpr int RING_DOUBLES = (16 + 10 + 8) * RING;
+constexpr int RING_DOUBLES = (16 + 12 + 8) * RING;
 constexpr int PRING = 66;                   // staged input pairs: chunk k (32 slots), chunk k+1 in flight, lane 31 of chunk k-1
 constexpr int XS_DOUBLES = XW * (RING_DOUBLES + 7 * PRING * 2);    // dynamic part (the math tables are static)
 
@@ -354,9 +359,9 @@ __device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* t
 // ---------------------------------------------------------------------------------------------------------------
 // y-sweep (a5): thread per column, register marching
 // ---------------------------------------------------------------------------------------------------------------
-constexpr int YT = 128;      // threads (columns) per block in k_ysweep
+constexpr int YT = 256;      // threads (columns) per block in k_ysweep: 2 blocks of 8 warps per SM (one table copy per block)
 constexpr int YST = 3;       // staged rows per thread: c-1 (re-read when its update starts), c, and c+1 in flight
-constexpr int YS_DOUBLES = (YST * 7 + 16 + 10) * YT + 16;       // dynamic part (+ 128 bytes of alignment slack; the math tables and the barriers are static)
+constexpr int YS_DOUBLES = (YST * 7 + 16 + 11) * YT + 16;       // dynamic part (+ 128 bytes of alignment slack; the math tables and the barriers are static)
 
 struct YPipe { int st, ph; };
 
@@ -373,11 +378,12 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
 {
     // staged input rows: per warp YST stages of [7 planes][32 columns], each filled by one bulk tensor copy;
     // thread-private slots, paired so that one 128-bit access moves two values: the window (W(c-1), 1/rho, rho c^2 and
-    // the 7 differences W(c-1) - W(c-2): 8 pairs), the previous right-face state (5 pairs)
+    // the 7 differences W(c-1) - W(c-2): 8 pairs), the previous right-face state (5 pairs + c)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double (*s_st)[7][32] = reinterpret_cast<double (*)[7][32]>(s_dyn + warp * (YST * 7 * 32));
     double2 (*s_w2)[YT] = reinterpret_cast<double2 (*)[YT]>(s_dyn + YST * 7 * YT);
     double2 (*s_r2)[YT] = reinterpret_cast<double2 (*)[YT]>(s_dyn + (YST * 7 + 16) * YT);
+    double* s_rc = s_dyn + (YST * 7 + 16 + 10) * YT;
     constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
     const int tid = threadIdx.x;
     bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
@@ -448,12 +454,12 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         {
             const double2 r0 = s_r2[0][tid], r1 = s_r2[1][tid], r2 = s_r2[2][tid], r3 = s_r2[3][tid], r4 = s_r2[4][tid];
             pr.r1 = r0.x; pr.r2 = r0.y; pr.un = r1.x; pr.ut = r1.y; pr.p = r2.x; pr.z1 = r2.y; pr.lam = r3.x; pr.rho = r3.y;
-            pr.rhoE = r4.x; pr.c = r4.y;
+            pr.xC = r4.x; pr.xD = r4.y; pr.c = s_rc[tid];
         }
         s_r2[0][tid] = make_double2(fr.r1, fr.r2); s_r2[1][tid] = make_double2(fr.un, fr.ut); s_r2[2][tid] = make_double2(fr.p, fr.z1);
-        s_r2[3][tid] = make_double2(fr.lam, fr.rho); s_r2[4][tid] = make_double2(fr.rhoE, fr.c);
+        s_r2[3][tid] = make_double2(fr.lam, fr.rho); s_r2[4][tid] = make_double2(fr.xC, fr.xD); s_rc[tid] = fr.c;
         double F[8];
-        hllc_fast(pr, fl, F);                     // face between cells c-2 and c-1
+        hllc_fast(P, pr, fl, F);                     // face between cells c-2 and c-1
         {                                         // finish cell c-2
             double o[7];
 #pragma unroll
@@ -489,10 +495,12 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
     // EDGE copy of the body: the 4 ramp-up rows, which run on a window / face / flux that is not real yet (finite or
     // not: nothing is stored or counted), and the last 3 rows, which stage and read the rows beyond the segment end -- ghost rows
     // when the segment ends at the grid's.  The rows in between touch cells of the grid only.
-    const int jmid = nrows - 3 > 4 ? nrows - 3 : 4;
-    for (int jj = 0; jj < 4; ++jj) row(std::true_type{}, jj);
-    for (int jj = 4; jj < jmid; ++jj) row(std::false_type{}, jj);
-    for (int jj = jmid; jj < nrows; ++jj) row(std::true_type{}, jj);
+    // (one call site per copy: a second one makes the compiler call the body instead of inlining it, and everything it captures
+    // -- the running update, the pipeline state -- then lives in local memory)
+    for (int jj = 0; jj < nrows; ++jj) {
+        if (jj < 4 || jj >= nrows - 3) row(std::true_type{}, jj);
+        else row(std::false_type{}, jj);
+    }
     pp.st = st; pp.ph = ph;                       // (a redo of the segment goes on from here: every staged row has been consumed)
     return hot;
 }
@@ -548,8 +556,8 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
     bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
     // rings of value PAIRS (one 128-bit access moves two values)
     double2* rw = reinterpret_cast<double2*>(s_ring + warp * RING_DOUBLES);   // [8][33]: W of the lane's cells A (0-6), B (7-13), 1/rho_B, (rho c^2)_B
-    double2* rfr = rw + 8 * RING;                    // [5][33]: right-face state of cell A
-    double2* rf = rfr + 5 * RING;                    // [4][33]: flux of face A-1/2
+    double2* rfr = rw + 8 * RING;                    // [6][33]: right-face state of cell A (11 values)
+    double2* rf = rfr + 6 * RING;                    // [4][33]: flux of face A-1/2
     double2* stg = reinterpret_cast<double2*>(s_dyn + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
     const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
@@ -655,7 +663,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             hot |= (oor1 && cnt1) || (oor2 && cnt2);
             rfr[0 * RING + sw] = make_double2(FR2.r1, FR2.r2); rfr[1 * RING + sw] = make_double2(FR2.un, FR2.ut);
             rfr[2 * RING + sw] = make_double2(FR2.p, FR2.z1);  rfr[3 * RING + sw] = make_double2(FR2.lam, FR2.rho);
-            rfr[4 * RING + sw] = make_double2(FR2.rhoE, FR2.c);
+            rfr[4 * RING + sw] = make_double2(FR2.xC, FR2.xD); rfr[5 * RING + sw] = make_double2(FR2.c, 0.0);
         }
         __syncwarp();
         // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
@@ -664,12 +672,12 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             FFace FRp;
             {
                 const double2 v0 = rfr[0 * RING + sr], v1 = rfr[1 * RING + sr], v2 = rfr[2 * RING + sr], v3 = rfr[3 * RING + sr];
-                const double2 v4 = rfr[4 * RING + sr];
+                const double2 v4 = rfr[4 * RING + sr], v5 = rfr[5 * RING + sr];
                 FRp.r1 = v0.x; FRp.r2 = v0.y; FRp.un = v1.x; FRp.ut = v1.y; FRp.p = v2.x; FRp.z1 = v2.y; FRp.lam = v3.x; FRp.rho = v3.y;
-                FRp.rhoE = v4.x; FRp.c = v4.y;
+                FRp.xC = v4.x; FRp.xD = v4.y; FRp.c = v5.x;
             }
-            hllc_fast(FRp, FL1, F1);
-            hllc_fast(FR1, FL2, F2);
+            hllc_fast(P, FRp, FL1, F1);
+            hllc_fast(P, FR1, FL2, F2);
 #pragma unroll
             for (int f = 0; f < 4; ++f) rf[f * RING + sw] = make_double2(F2[2 * f], F2[2 * f + 1]);
         }
@@ -888,7 +896,7 @@ void launch_sweep_fused(const Params& P, const double* qin, const CUtensorMap* t
         sweep_dispatch(false, 0, mode, lim, dim3(lines, (P.nx + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg, end_step && mode >= MODE_TRAIL ? 1 : 0);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
-        const int seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 2.6);
+        const int seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 1.3);
         sweep_dispatch(false, 1, mode, lim, dim3(lines, (P.ny + seg - 1) / seg), s, pdl, P, qin, tm_in, qout, dtp, ctl, seg, end_step && mode >= MODE_TRAIL ? 1 : 0);
     }
 }
@@ -902,7 +910,7 @@ void sweep_geometry(const Params& P, int dir, int* seg, int* ramp, long long* nb
         *nblocks = (long long)lines * ((P.nx + *seg - 1) / *seg);
     } else {
         const int lines = (P.nx + YT - 1) / YT;
-        *seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 2.6); *ramp = 4;
+        *seg = pick_seg(P.ny, 128, 4, 1.5, lines, num_sms(), NMSDT_Y_MINBLOCKS, 1.3); *ramp = 4;
         *nblocks = (long long)lines * ((P.ny + *seg - 1) / *seg);
     }
 }

@@ -534,7 +534,7 @@ def test_sweep_geometry_covers_the_grid(B, name, kw):
     cfg = inputs.config(name, **kw)
     g = cfg["grid"]
     s = B.Sim(g, cfg["eos"], cfg["kin"])
-    for d, (n, lines) in enumerate(((g["nx"], (g["ny"] + 3) // 4), (g["ny"], (g["nx"] + 127) // 128))):
+    for d, (n, lines) in enumerate(((g["nx"], (g["ny"] + 3) // 4), (g["ny"], (g["nx"] + 255) // 256))):
         seg, ramp, nb = s.sweep_geometry(d)
         assert seg >= 1 and ramp == 4 and nb == lines * ((n + seg - 1) // seg)
         if d == 0:
