@@ -32,11 +32,22 @@ namespace {
 enum { MODE_PLAIN = 0, MODE_LEAD = 1, MODE_TRAIL = 2, MODE_TRAIL_INERT = 3 };
 
 // A face state: the reconstructed primitives, the mixture density and sound speed -- what both sides of a face need for the wave
-// speeds -- and (x^C, x^D) of its liquid density.  The total energy is NOT formed here: only the side the HLLC fan selects needs
-// it, so hllc_fast forms it after the selection from (x^C, x^D) (11 FP64 instructions per face state moved to 12 per face).
-struct FFace { double r1, r2, un, ut, p, z1, lam, rho, c, xC, xD; };
+// speeds -- and either the total energy or (x^C, x^D) of its liquid density.  Only the side the HLLC fan selects needs the total
+// energy, so with DEFER hllc_fast forms it after the selection from (x^C, x^D): 11 FP64 instructions per face state become 12
+// per face (-10 per cell and pass).  The price is a longer dependency chain inside the flux; every sweep kernel takes it
+// (-1.8 ... -2.8 % each) except k_xsweep<TRAIL>, which runs 12 warps per SM with its trailing source chains already latency
+// bound and got 1.1 % slower with it: that one forms the energy with the face state as before.
+struct FFace { double r1, r2, un, ut, p, z1, lam, rho, c, rhoE, xC, xD; };
 
-template <bool EX>
+// E(rho1, rho2, z1, p) + kinetic energy (O4.3): Eq. 3-4 enter through (p - p_ref2)/Gamma2 + rho2 e_ref2 = p/Gamma2 + E1 x^C + E2 x^D - E3 x
+__device__ __forceinline__ double face_energy(const Params& P, double r2, double un, double ut, double p, double z1, double rho, double xC, double xD)
+{
+    const double brk = fma(p, P.iG2, fma(P.E1, xC, fma(P.E2, xD, -P.E3 * (r2 * P.irho02))));
+    const double kin = 0.5 * rho * fma(un, un, ut * ut);
+    return fma(z1 * P.iG1, p, fma(1.0 - z1, brk, kin));
+}
+
+template <bool EX, bool DEFER>
 __device__ __forceinline__ void face_fast(const Params& P, const double* __restrict__ tab, const double W[7], FFace& f, bool& oor)
 {
     const double z1 = W[5], z2 = 1.0 - z1, p = W[4];
@@ -47,6 +58,7 @@ __device__ __forceinline__ void face_fast(const Params& P, const double* __restr
     double xC, xD;
     eos_pow<EX>(P, tab, x, xC, xD, oor);
     f.xC = xC; f.xD = xD;
+    f.rhoE = DEFER ? 0.0 : face_energy(P, W[1], W[2], W[3], p, z1, rho, xC, xD);
     // Eq. 3-4 enter the sound speed through rho2 c2^2 = (Gamma2+1) p + R1 x^C + R2 x^D (O2)
     const double xi = fma(z1, P.iG1, z2 * P.iG2);
     const double r2c22 = fma(P.R1, xC, fma(P.R2, xD, P.G2p1 * p));
@@ -124,6 +136,7 @@ __device__ __forceinline__ void recon_fast(const Params& P, const FCell& Wm, con
 }
 
 // O4.4-5: HLLC flux F[0..6] (component 2 = normal momentum), F[7] = face velocity
+template <bool DEFER>
 __device__ __forceinline__ void hllc_fast(const Params& P, const FFace& L, const FFace& R, double F[8])
 {
     const double SL = dmin_(L.un - L.c, R.un - R.c);                  // R9: Davis
@@ -138,12 +151,10 @@ __device__ __forceinline__ void hllc_fast(const Params& P, const FFace& L, const
     const bool star = sl_neg && sr_pos;
     const double r1 = useL ? L.r1 : R.r1, r2 = useL ? L.r2 : R.r2, un = useL ? L.un : R.un, ut = useL ? L.ut : R.ut;
     const double p = useL ? L.p : R.p, z1 = useL ? L.z1 : R.z1, lam = useL ? L.lam : R.lam;
-    const double rho = useL ? L.rho : R.rho, xC = useL ? L.xC : R.xC, xD = useL ? L.xD : R.xD, SK = useL ? SL : SR;
-    // total energy of the selected side (O4.3): Eq. 3-4 enter through (p - p_ref2)/Gamma2 + rho2 e_ref2 = p/Gamma2 + E1 x^C + E2 x^D - E3 x
-    const double z2 = 1.0 - z1;
-    const double brk = fma(p, P.iG2, fma(P.E1, xC, fma(P.E2, xD, -P.E3 * (r2 * P.irho02))));
-    const double kin = 0.5 * rho * fma(un, un, ut * ut);
-    const double rhoE = fma(z1 * P.iG1, p, fma(z2, brk, kin));
+    const double rho = useL ? L.rho : R.rho, SK = useL ? SL : SR;
+    double rhoE;                                                       // total energy of the selected side
+    if (DEFER) rhoE = face_energy(P, r2, un, ut, p, z1, rho, useL ? L.xC : R.xC, useL ? L.xD : R.xD);
+    else rhoE = useL ? L.rhoE : R.rhoE;
     // chi = (SK-un)/(SK-S*) and p/(SK-un) from one reciprocal; outside the fan SKs = 0 and the star terms vanish
     const double a = SK - un, b = SK - Sstar;
     const double rab = star ? q_rcp(a * b) : 0.0;
@@ -153,7 +164,7 @@ __device__ __forceinline__ void hllc_fast(const Params& P, const FFace& L, const
     // U*_k = chi U_k for the advected components, so F_k = U_k un + SK (chi - 1) U_k = U_k u_face with the
     // HLLC-consistent face velocity u_face = un + SK (chi - 1) (R8)
     const double uf = fma(SKs, chi - 1.0, un);
-    const double U0 = z1 * r1, U1 = z2 * r2;
+    const double U0 = z1 * r1, U1 = (1.0 - z1) * r2;
     F[0] = U0 * uf;
     F[1] = U1 * uf;
     F[2] = fma(rho * un, un, p) + SKs * rho * fma(chi, Sstar, -un);
@@ -448,8 +459,8 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         }
         FFace fl, fr, pr;
         bool oor = false;                         // a face density outside the power tables (only counted once the window is real)
-        face_fast<EXACT>(P, s_tab, WL, fl, oor);
-        face_fast<EXACT>(P, s_tab, WR, fr, oor);
+        face_fast<EXACT, true>(P, s_tab, WL, fl, oor);
+        face_fast<EXACT, true>(P, s_tab, WR, fr, oor);
         hot |= oor && (!EDGE || jj >= 2);
         {
             const double2 r0 = s_r2[0][tid], r1 = s_r2[1][tid], r2 = s_r2[2][tid], r3 = s_r2[3][tid], r4 = s_r2[4][tid];
@@ -459,7 +470,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
         s_r2[0][tid] = make_double2(fr.r1, fr.r2); s_r2[1][tid] = make_double2(fr.un, fr.ut); s_r2[2][tid] = make_double2(fr.p, fr.z1);
         s_r2[3][tid] = make_double2(fr.lam, fr.rho); s_r2[4][tid] = make_double2(fr.xC, fr.xD); s_rc[tid] = fr.c;
         double F[8];
-        hllc_fast(P, pr, fl, F);                     // face between cells c-2 and c-1
+        hllc_fast<true>(P, pr, fl, F);                     // face between cells c-2 and c-1
         {                                         // finish cell c-2
             double o[7];
 #pragma unroll
@@ -552,6 +563,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr int SRC = (MODE == MODE_LEAD || MODE == MODE_TRAIL) ? (EXACT ? SRC_EXACT : SRC_FAST) : SRC_NONE;
+    constexpr bool XDEFER = MODE != MODE_TRAIL;         // (see FFace)
     double* s_ring = s_dyn;
     bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
     // rings of value PAIRS (one 128-bit access moves two values)
@@ -654,16 +666,16 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             const bool cnt1 = !EDGE || (real && A - 1 <= P.nx), cnt2 = !EDGE || (real && A <= P.nx);
             bool oor1 = false, oor2 = false;         // a face density outside the power tables
             recon_fast<LIM, EXACT>(P, Wmm, Wm1, WA, khalf, WL, WR, cnt1, hot);
-            face_fast<EXACT>(P, s_tab, WL, FL1, oor1);
-            face_fast<EXACT>(P, s_tab, WR, FR1, oor1);
+            face_fast<EXACT, XDEFER>(P, s_tab, WL, FL1, oor1);
+            face_fast<EXACT, XDEFER>(P, s_tab, WR, FR1, oor1);
             recon_fast<LIM, EXACT>(P, Wm1, WA, WB, khalf, WL, WR, cnt2, hot);
-            face_fast<EXACT>(P, s_tab, WL, FL2, oor2);
+            face_fast<EXACT, XDEFER>(P, s_tab, WL, FL2, oor2);
             FFace FR2;
-            face_fast<EXACT>(P, s_tab, WR, FR2, oor2);
+            face_fast<EXACT, XDEFER>(P, s_tab, WR, FR2, oor2);
             hot |= (oor1 && cnt1) || (oor2 && cnt2);
             rfr[0 * RING + sw] = make_double2(FR2.r1, FR2.r2); rfr[1 * RING + sw] = make_double2(FR2.un, FR2.ut);
             rfr[2 * RING + sw] = make_double2(FR2.p, FR2.z1);  rfr[3 * RING + sw] = make_double2(FR2.lam, FR2.rho);
-            rfr[4 * RING + sw] = make_double2(FR2.xC, FR2.xD); rfr[5 * RING + sw] = make_double2(FR2.c, 0.0);
+            rfr[4 * RING + sw] = XDEFER ? make_double2(FR2.xC, FR2.xD) : make_double2(FR2.rhoE, 0.0); rfr[5 * RING + sw] = make_double2(FR2.c, 0.0);
         }
         __syncwarp();
         // ---- phase 3: faces A-3/2 and A-1/2 ---------------------------------------------------------------------
@@ -674,10 +686,10 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
                 const double2 v0 = rfr[0 * RING + sr], v1 = rfr[1 * RING + sr], v2 = rfr[2 * RING + sr], v3 = rfr[3 * RING + sr];
                 const double2 v4 = rfr[4 * RING + sr], v5 = rfr[5 * RING + sr];
                 FRp.r1 = v0.x; FRp.r2 = v0.y; FRp.un = v1.x; FRp.ut = v1.y; FRp.p = v2.x; FRp.z1 = v2.y; FRp.lam = v3.x; FRp.rho = v3.y;
-                FRp.xC = v4.x; FRp.xD = v4.y; FRp.c = v5.x;
+                FRp.xC = v4.x; FRp.xD = v4.y; FRp.rhoE = v4.x; FRp.c = v5.x;
             }
-            hllc_fast(P, FRp, FL1, F1);
-            hllc_fast(P, FR1, FL2, F2);
+            hllc_fast<XDEFER>(P, FRp, FL1, F1);
+            hllc_fast<XDEFER>(P, FR1, FL2, F2);
 #pragma unroll
             for (int f = 0; f < 4; ++f) rf[f * RING + sw] = make_double2(F2[2 * f], F2[2 * f + 1]);
         }
