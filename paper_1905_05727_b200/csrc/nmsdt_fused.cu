@@ -341,17 +341,18 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // barrier with the byte count and issues one bulk tensor copy per row -- a {32 columns, 1 row, 7 planes} box of the
 // plane set (described by a CUtensorMap built in sim_create) -- instead of 7 cp.async + their 64-bit address
 // arithmetic in every thread.
+// (The helpers take 32-bit shared-space addresses: converting a generic pointer at every use costs ~18 instructions per row.)
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
+__device__ __forceinline__ void mbar_init(unsigned bar, int count)
 {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, int bytes)
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, int bytes)
 {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, int parity)
+__device__ __forceinline__ void mbar_wait(unsigned bar, int parity)
 {
     asm volatile(
         "{\n"
@@ -359,12 +360,12 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, int parity)
         "WAIT_%=:\n"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
         "@!p bra WAIT_%=;\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned long long* bar)
+__device__ __forceinline__ void tma_load_3d(unsigned smem_dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned bar)
 {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(smem_u32(smem_dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+                 ::"r"(smem_dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -385,7 +386,7 @@ struct YPipe { int st, ph; };
 // the pass is out of place).
 template <int MODE, bool EXACT, int LIM>
 __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ qout, const double* __restrict__ dtp, int seg, int col, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad,
-                                          const CUtensorMap* tm, unsigned long long* bars, unsigned wmask, YPipe& pp)
+                                          const CUtensorMap* tm, unsigned bars, unsigned wmask, YPipe& pp)
 {
     // staged input rows: per warp YST stages of [7 planes][32 columns], each filled by one bulk tensor copy;
     // thread-private slots, paired so that one 128-bit access moves two values: the window (W(c-1), 1/rho, rho c^2 and
@@ -408,12 +409,13 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
     // `r` is the row of the grid, -2 .. ny + 1; a ghost row (only ever staged and read by the EDGE copy of the body) is taken
     // from the interior row the boundary rule names (ghost_src), its normal momentum negated on read where the wall reflects.
     const int tx = NGX + col - lane;
+    const unsigned st_addr = smem_u32(&s_st[0][0][0]);    // shared-space addresses of the warp's stages (1792 B each) and barriers
     auto stage_row = [&](int sg, int r, bool edge) {
         if (lane == 0) {
             bool flip;
             const int src = edge ? ghost_src(r, P.ny, P.bc_ylo, P.bc_yhi, flip) : -1;
-            mbar_expect_tx(&bars[sg], 7 * 32 * (int)sizeof(double));
-            tma_load_3d(&s_st[sg][0][0], tm, tx, (src >= 0 ? src : r) + NGY, 0, &bars[sg]);
+            mbar_expect_tx(bars + 8u * sg, 7 * 32 * (int)sizeof(double));
+            tma_load_3d(st_addr + (unsigned)(7 * 32 * sizeof(double)) * sg, tm, tx, (src >= 0 ? src : r) + NGY, 0, bars + 8u * sg);
         }
     };
     auto read_row = [&](int sg, double q[7]) {            // sweep field order: q0, q1, q3 (normal), q2 (tangential), q4, q5, q6
@@ -431,7 +433,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
             __syncwarp(wmask);                    // every lane is done with stage sn (row jj - 2, last read in the previous iteration)
             stage_row(sn, c0 - 1 + jj, EDGE);
         }
-        mbar_wait(&bars[st], ph);
+        mbar_wait(bars + 8u * st, ph);
         FCell Wp;
         {
             double q[7];
@@ -528,7 +530,7 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
     __shared__ __align__(8) unsigned long long s_bar[YT / 32][YST];
     pdl_launch_dependents();
     for (int i = threadIdx.x; i < MATH_TAB_DOUBLES; i += blockDim.x) s_tab[i] = P.tab[i];
-    if (threadIdx.x < (YT / 32) * YST) mbar_init(&s_bar[0][0] + threadIdx.x, 1);
+    if (threadIdx.x < (YT / 32) * YST) mbar_init(smem_u32(&s_bar[0][0] + threadIdx.x), 1);
     fence_proxy_async();
     __syncthreads();
     pdl_wait();                                                  // the state, dt and the control block belong to the previous kernel until here
@@ -537,7 +539,7 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
     double smax = 0.0; int bad = 0;
     if (col < P.nx) {
         YPipe pp{0, 0};
-        unsigned long long* bars = s_bar[threadIdx.x >> 5];
+        const unsigned bars = smem_u32(s_bar[threadIdx.x >> 5]);
         const bool redo = y_segment<MODE, false, LIM>(P, qout, dtp, seg, col, s_tab, s_dyn, smax, bad, &tm, bars, wmask, pp);
         if (__any_sync(wmask, redo)) {                           // rare: redo the warp's segment with the exact R13 / R17 rules
             if ((threadIdx.x & 31) == 0) atomicAdd(&ctl->redo, 1);
