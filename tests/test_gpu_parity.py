@@ -544,3 +544,29 @@ def test_sweep_geometry_covers_the_grid(B, name, kw):
         if name in ("C1",) and not kw:
             assert nb <= 148 * 4 and seg <= (60 if d == 0 else 4)
     s.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("nx,ny,bcx,bcy", [(8, 8, 1, 1), (2, 2, 1, 1), (2, 3, 0, 2), (5, 1, 2, 1), (1, 6, 0, 0), (63, 2, 3, 1), (66, 4, 2, 2)])
+def test_tiny_grids(O, B, nx, ny, bcx, bcy, variant):
+    """grids smaller than one chunk / one segment, down to a single row or column: every cell's stencil reaches a ghost cell, so
+    the boundary rules folded into the sweeps (periodic wrap of 1- and 2-cell lines, mirror images, fixed inflow) carry the result"""
+    bx = (bcx, bcx if bcx != 3 else 0)
+    grid = dict(nx=nx, ny=ny, dx=4e-6, dy=4e-6, bc_xlo=bx[0], bc_xhi=bx[1], bc_ylo=bcy, bc_yhi=bcy, cfl=0.4, limiter=0)
+    rng = np.random.default_rng(100 * nx + ny)
+    e = O.make_eos(inputs.EOS)
+    q = np.empty((7, ny, nx))
+    for j in range(ny):
+        for i in range(nx):
+            W = [1.2 * rng.uniform(1, 30), 1134.0 * rng.uniform(1.0, 1.6), rng.uniform(-800, 800), rng.uniform(-800, 800),
+                 10 ** rng.uniform(5, 9.9), rng.choice([1e-6, 0.3, 1 - 1e-6]), rng.uniform(0.2, 1.0)]
+            q[:, j, i] = O.prim_to_cons(e, np.array(W))
+    o = O.Oracle(grid, inputs.EOS, inputs.KIN)
+    o.init_fields(list(q))
+    s = B.Sim(grid, inputs.EOS, inputs.KIN, variant=variant)
+    s.init_fields(list(q))
+    for it in range(4):
+        dt = 0.5 * o.cfl_dt()
+        o.step_dt(1, dt), s.step_dt(1, dt)
+        _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="tiny %dx%d bc %d/%d step %d" % (nx, ny, bcx, bcy, it))
+    assert s.diagnostics()["bad_state"] == 0
