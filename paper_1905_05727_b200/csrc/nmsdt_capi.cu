@@ -70,8 +70,8 @@ struct sim {
     double phi_target = 0.0, phi_achieved = 0.0;    // seeded generator: air fraction asked for / placed (0 without a generator)
     int variant = SIM_VARIANT_FUSED;
     int use_graph = 1;
-    int use_pdl = 0;                // chain the step's five kernels by programmatic dependent launch (measured slower: off)
-    cudaGraphExec_t gexec = nullptr;    // fused path: one even (X-Y) + one odd (Y-X) step = 10 kernel nodes
+    int use_pdl = 0;                // chain the kernels of sim_step by programmatic dependent launch (measured slower: off)
+    cudaGraphExec_t gexec = nullptr;    // fused path: one even (X-Y) + one odd (Y-X) step = 4 kernel nodes
     cudaStream_t cap_stream = nullptr;  // private stream the graph is captured on (the caller's may be the legacy stream)
     bool graph_failed = false;
     bool cfl_valid = false;         // fused path: ctl->dt / ctl->tsafe describe the current state and dt mode
