@@ -570,3 +570,25 @@ def test_tiny_grids(O, B, nx, ny, bcx, bcy, variant):
         o.step_dt(1, dt), s.step_dt(1, dt)
         _assert_one_step(o, s, tol=(it + 1) * TOL_ONE_STEP, what="tiny %dx%d bc %d/%d step %d" % (nx, ny, bcx, bcy, it))
     assert s.diagnostics()["bad_state"] == 0
+
+
+def test_launch_modes_change_nothing_but_timing(B):
+    """sim_set_launch_mode: CUDA-graph replay and programmatic dependent launch reorder when kernels start, never what they
+    compute: 11 steps (odd: the graph path replays pairs and enqueues the rest) give bit-identical states in all four modes"""
+    cfg = inputs.config("C4", nx=640, ny=160, p_shock=9e9)
+    ref = None
+    for use_graph in (True, False):
+        for use_pdl in (False, True):
+            s = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=1)
+            s.set_launch_mode(use_graph=use_graph, use_pdl=use_pdl)
+            s.init(cfg["init"])
+            s.step(4)
+            s.step(7)
+            q = s.state()
+            d = s.diagnostics()
+            assert d["step"] == 11 and d["bad_state"] == 0
+            if ref is None:
+                ref = (q, d)
+            else:
+                assert all(np.array_equal(a, b) for a, b in zip(q, ref[0])) and d == ref[1], (use_graph, use_pdl)
+            s.close()
