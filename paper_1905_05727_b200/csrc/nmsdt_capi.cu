@@ -355,6 +355,7 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     sim* s = new sim();
     s->g = *g; s->e = *e; s->k = *k;
     s->L = make_layout(g->nx, g->ny);
+    if (s->L.fstride >= (1LL << 32)) { delete s; return fail(nullptr, SIM_ERR_ARG, "sim_create: a plane of 2^32 doubles or more (34 GB) is not supported"); }
     s->stream = (cudaStream_t)cuda_stream;
     if (device_buf) {
         if (bytes < s->L.total || ((uintptr_t)device_buf & 255)) { delete s; return fail(nullptr, SIM_ERR_ARG, "sim_create: device_buf too small or not 256-byte aligned"); }

@@ -337,6 +337,17 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// p + bytes as ONE 64-bit add the compiler may not take apart.  Left to itself it rebuilds every plane's address from a 64-bit
+// element index (add, add-with-carry, shift-and-add, twice) -- 4-5 instructions per address, 7 addresses per load and per
+// store; a chain of these costs 2 per address.
+template <typename T>
+__device__ __forceinline__ T* ptr_add(T* p, unsigned long long bytes)
+{
+    unsigned long long r;
+    asm("add.u64 %0, %1, %2;" : "=l"(r) : "l"((unsigned long long)p), "l"(bytes));
+    return (T*)r;
+}
+
 // TMA (cp.async.bulk.tensor) + mbarrier primitives of the y-sweep's input staging: one lane per warp arms the stage's
 // barrier with the byte count and issues one bulk tensor copy per row -- a {32 columns, 1 row, 7 planes} box of the
 // plane set (described by a CUtensorMap built in sim_create) -- instead of 7 cp.async + their 64-bit address
@@ -402,7 +413,11 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
     const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
     const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
-    const long long fs = P.fstride, pitch = P.pitch;
+    // (the plane stride as a 32-bit number -- sim_create refuses planes of 2^32 doubles -- so that a plane's address is ONE
+    // IMAD.WIDE.U32 from the row pointer instead of a 64 x 64-bit product)
+    const unsigned long long fs = (unsigned)P.fstride, fsb = fs * sizeof(double);
+    const long long pitch = P.pitch;
+    const unsigned long long pitchb = (unsigned long long)pitch * sizeof(double);
     double* pout = qout + (long long)(c0 + NGY) * pitch + NGX + col;
     const int nrows = c1 - c0 + 4;
     // one lane per warp stages a row: the {32, 1, 7} box at (first column of the warp, row, plane 0) of the input plane set.
@@ -488,9 +503,10 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
                 hot |= valid && hot1;
             }
             if (valid) {
-                pout[0] = o[0]; pout[fs] = o[1]; pout[3 * fs] = o[2]; pout[2 * fs] = o[3]; pout[4 * fs] = o[4]; pout[5 * fs] = o[5];
-                pout[6 * fs] = o[6];
-                pout += pitch;
+                double* po = pout;                // planes 0 .. 6 hold q0, q1, q2 (tangential here), q3 (normal), q4, q5, q6
+                *po = o[0]; po = ptr_add(po, fsb); *po = o[1]; po = ptr_add(po, fsb); *po = o[3]; po = ptr_add(po, fsb); *po = o[2];
+                po = ptr_add(po, fsb); *po = o[4]; po = ptr_add(po, fsb); *po = o[5]; po = ptr_add(po, fsb); *po = o[6];
+                pout = ptr_add(pout, pitchb);
             }
         }
         {                                         // start cell c-1 with its lower-face flux
@@ -576,7 +592,8 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
     const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
     const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
-    const long long fs = P.fstride;
+    const unsigned long long fs = (unsigned)P.fstride;     // (32-bit plane stride: see y_segment)
+    const unsigned long long fsb = fs * sizeof(double);
     const double* rin = qin + (long long)(row + NGY) * P.pitch + NGX;
     double* rout = qout + (long long)(row + NGY) * P.pitch + NGX;
     const int nxe = (P.nx + 1) & ~1;                 // last pair base that is ever needed (cell nx+1 is the outer ghost; for odd nx the pair ends in row padding)
@@ -604,9 +621,9 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
         FCell WA, WB;
         const int psn = ps + 32 >= PRING ? ps + 32 - PRING : ps + 32;
         if (k + 1 < niter) {                         // stage the next chunk while this one is computed
-            const int An = min(A + 64, nxe);
+            const double* gp = rin + min(A + 64, nxe);      // one 64-bit pointer, then a chain of plane strides
 #pragma unroll
-            for (int f = 0; f < 7; ++f) cp_async16(reinterpret_cast<double*>(stg + f * PRING + psn), rin + An + f * fs);
+            for (int f = 0; f < 7; ++f, gp = ptr_add(gp, fsb)) cp_async16(reinterpret_cast<double*>(stg + f * PRING + psn), gp);
         }
         cp_async_commit();
         cp_async_wait<1>();
@@ -732,7 +749,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
             double* po = rout + u0;
             if (valid) {
 #pragma unroll
-                for (int f = 0; f < 7; ++f) *reinterpret_cast<double2*>(po + f * fs) = make_double2(oa[f], ob[f]);
+                for (int f = 0; f < 7; ++f, po = ptr_add(po, fsb)) *reinterpret_cast<double2*>(po) = make_double2(oa[f], ob[f]);
             }
         }
         sw = sw == 0 ? RING - 1 : sw - 1;            // (32 (k+1) + lane) mod 33
