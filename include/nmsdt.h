@@ -162,6 +162,26 @@ int sim_redo_count(sim_t*, long long* n);
 int sim_profiles(sim_t*, double p_front, double* host_pbar, double* host_rhobar, double* host_ubar, double* xs_out);
 int sim_qdot_pdf(sim_t*, double n_lo, double dn, int nbins, double* host_mass, long long* host_count);
 int sim_shock_kinematics(sim_t*, const double* host_t, const double* host_xs, int n, double dtau, double* host_us, double* host_as);
+/* sim_qdot_pdf for callers that must not touch the CUDA heap.  Same arguments, same kernels, same launch shape and
+ * therefore bit-for-bit the same histogram as sim_qdot_pdf (Eq. 14-16), but the device scratch is a fixed
+ * array inside libnmsdt.so's device image (about 2.3 MiB) instead of a buffer the handle grows with cudaMalloc.
+ *   Meant for: (1) hosts that gave the whole GPU to their own arena and lend this library its workspace through
+ *   sim_create's device_buf -- nothing is left for cudaMalloc to hand out, so sim_qdot_pdf fails there; (2) in-situ
+ *   monitors that sample the histogram every few steps while other handles have sim_step work queued: cudaMalloc and
+ *   cudaFree synchronise the whole device and would stall those queues at every sample.
+ *   Limit: 1 <= nbins <= 512 (the paper's window has 400 bins); more returns SIM_ERR_ARG and sim_last_error names the
+ *   limit.  The price: every GPU on which the library's kernels get loaded holds those 2.3 MiB until the process exits.
+ *   This call, including its error paths, calls no cudaMalloc / cudaFree and no library routine that allocates device
+ *   memory; host_mass / host_count are HOST arrays of nbins entries owned by the caller (either may be NULL) and are
+ *   filled by plain device-to-host copies on the handle's stream.
+ *   Set-up: the FIRST call on each device looks up the array's address on that device (cudaGetSymbolAddress) and raises
+ *   the histogram kernel's shared-memory limit there; the device that holds the handle's state must be the current
+ *   device (SIM_ERR_ARG otherwise).  Make that first call before starting any stream capture in the process.
+ *   Sharing: there is ONE array per device, shared by all handles and all host threads, and it keeps the last call's
+ *   contents (the call clears the part that has to start at zero itself).  Calls whose GPU work can overlap -- two
+ *   handles on different streams of one device, from one thread or several -- race on it and return garbage; serialise
+ *   them.  Calls on one handle are ordered by its stream and this call is [sync], so a single handle needs no care. */
+int sim_qdot_pdf_noalloc(sim_t*, double n_lo, double dn, int nbins, double* host_mass, long long* host_count);
 
 /* ---- multi-GPU slab decomposition along x (the paper names multi-GPU runs as future
  * work).  The domain is cut into slabs of whole columns, one handle (one GPU, one process) per slab.  A side

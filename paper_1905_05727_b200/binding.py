@@ -23,6 +23,7 @@ SYMBOLS = ["sim_workspace_bytes", "sim_create", "sim_destroy", "sim_last_error",
            "sim_cfl_dt", "sim_step", "sim_step_dt", "sim_halo", "sim_sweep", "sim_source", "sim_diagnostics",
            "sim_read_field", "sim_get_cavities", "sim_cavity_stats", "sim_redo_count", "sim_set_variant", "sim_set_launch_mode", "sim_sweep_geometry", "sim_launch_count", "sim_device_layout",
            "sim_probe_fp64", "sim_probe_issue", "sim_probe_math", "sim_profile", "sim_kernel_time", "sim_profiles", "sim_qdot_pdf",
+           "sim_qdot_pdf_noalloc",
            "sim_shock_kinematics", "sim_init_slab", "sim_slab_halo_bytes", "sim_slab_begin", "sim_slab_smax_ptr",
            "sim_slab_ctl", "sim_slab_pass_dir", "sim_slab_pass", "sim_slab_pack", "sim_slab_unpack", "sim_slab_info",
            "sim_slab_connect", "sim_slab_push", "sim_slab_ipc_export", "sim_slab_ipc_open", "sim_slab_ipc_close"]
@@ -117,6 +118,7 @@ def load_library():
         "sim_probe_issue": (C.c_int, [vp, dp]),
         "sim_profiles": (C.c_int, [vp, C.c_double, dp, dp, dp, dp]),
         "sim_qdot_pdf": (C.c_int, [vp, C.c_double, C.c_double, C.c_int, dp, C.POINTER(C.c_longlong)]),
+        "sim_qdot_pdf_noalloc": (C.c_int, [vp, C.c_double, C.c_double, C.c_int, dp, C.POINTER(C.c_longlong)]),
         "sim_shock_kinematics": (C.c_int, [vp, dp, dp, C.c_int, C.c_double, dp, dp]),
         "sim_probe_math": (C.c_int, [vp, C.c_int, dp, C.c_int, C.c_double, C.c_double, dp, dp]),
         "sim_profile": (C.c_int, [vp, C.c_int]),
@@ -334,6 +336,17 @@ class Sim:
         c = np.empty(nbins, dtype=np.int64)
         self._chk(self.L.sim_qdot_pdf(self.h, float(n_lo), float(dn), int(nbins), m.ctypes.data_as(C.POINTER(C.c_double)),
                                       c.ctypes.data_as(C.POINTER(C.c_longlong))), "sim_qdot_pdf")
+        return m, c
+
+    def qdot_pdf_noalloc(self, n_lo=2.0, dn=0.02, nbins=400):
+        """Eq. 14-16 as qdot_pdf, for callers that cannot let the library allocate device memory (the GPU belongs to the
+        caller's own arena, or a cudaMalloc's device-wide synchronisation would stall work queued by other handles): the
+        scratch is a fixed array inside libnmsdt.so, so nbins <= 512, and calls that may overlap on one GPU must be
+        serialised by the caller (include/nmsdt.h: sim_qdot_pdf_noalloc).  Returns (mass[nbins], count[nbins])."""
+        m = np.empty(nbins, dtype=np.float64)
+        c = np.empty(nbins, dtype=np.int64)
+        self._chk(self.L.sim_qdot_pdf_noalloc(self.h, float(n_lo), float(dn), int(nbins), m.ctypes.data_as(C.POINTER(C.c_double)),
+                                              c.ctypes.data_as(C.POINTER(C.c_longlong))), "sim_qdot_pdf_noalloc")
         return m, c
 
     def shock_kinematics(self, t, xs, dtau):

@@ -914,6 +914,28 @@ int sim_qdot_pdf(sim_t* s, double n_lo, double dn, int nbins, double* host_mass,
     return check_cuda(s, "sim_qdot_pdf");
 }
 
+int sim_qdot_pdf_noalloc(sim_t* s, double n_lo, double dn, int nbins, double* host_mass, long long* host_count)
+{
+    if (!s || !(dn > 0.0) || nbins < 1) return fail(s, SIM_ERR_ARG, "sim_qdot_pdf_noalloc: bad argument (nbins >= 1, dn > 0)");
+    if (nbins > POST_NOALLOC_MAX_BINS)
+        return fail(s, SIM_ERR_ARG, "sim_qdot_pdf_noalloc: nbins = " + std::to_string(nbins) + " exceeds the " + std::to_string(POST_NOALLOC_MAX_BINS) +
+                                    " bins of the library's static scratch; use sim_qdot_pdf (which allocates) for wider windows");
+    if (!s->inited) return fail(s, SIM_ERR_STATE, "sim_qdot_pdf_noalloc: not initialised");
+    if (!s->P.reactive) {                       // inert run: no energy release, empty statistics (as sim_qdot_pdf)
+        for (int b = 0; b < nbins; ++b) { if (host_mass) host_mass[b] = 0.0; if (host_count) host_count[b] = 0; }
+        return SIM_OK;
+    }
+    double* d_mass = nullptr; unsigned long long* d_count = nullptr;
+    const char* why = "";
+    const int n = launch_qdot_hist_noalloc(s->P, s->A, n_lo, dn, nbins, &d_mass, &d_count, s->stream, &why);
+    if (n < 0) return fail(s, n == -1 ? SIM_ERR_ARG : SIM_ERR_CUDA, std::string("sim_qdot_pdf_noalloc: ") + why);
+    s->launches += n;
+    if (host_mass) cudaMemcpyAsync(host_mass, d_mass, sizeof(double) * nbins, cudaMemcpyDeviceToHost, s->stream);
+    if (host_count) cudaMemcpyAsync(host_count, d_count, sizeof(long long) * nbins, cudaMemcpyDeviceToHost, s->stream);
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return check_cuda(s, "sim_qdot_pdf_noalloc");
+    return check_cuda(s, "sim_qdot_pdf_noalloc");
+}
+
 int sim_shock_kinematics(sim_t* s, const double* host_t, const double* host_xs, int n, double dtau, double* host_us, double* host_as)
 {
     if (!s || !host_t || !host_xs || !host_us || !host_as || n < 2 || !(dtau > 0.0)) return fail(s, SIM_ERR_ARG, "sim_shock_kinematics: bad argument");

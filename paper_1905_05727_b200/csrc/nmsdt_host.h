@@ -68,6 +68,10 @@ int launch_profiles(const Params& P, const double* q, double p_front, double* bu
 int launch_qdot_hist(const Params& P, const double* q, double n_lo, double dn, int nbins, double* buf, double** d_mass,
                      unsigned long long** d_count, cudaStream_t s);
 int launch_kinematics(const double* d_t, const double* d_xs, int n, double dtau, double* d_us, double* d_as, cudaStream_t s);
+// sim_qdot_pdf_noalloc: the same two kernels on a fixed __device__ array of nmsdt_post.cu (no heap); -1 / -2 + *why on error
+constexpr int POST_NOALLOC_MAX_BINS = 512;
+int launch_qdot_hist_noalloc(const Params& P, const double* q, double n_lo, double dn, int nbins, double** d_mass, unsigned long long** d_count,
+                             cudaStream_t s, const char** why);
 
 // slab decomposition (nmsdt_slab.cu): a block of 7 planes x ny rows x 2 columns inside some strided layout
 struct SlabView { double* base; long long fstride; long long pitch; };

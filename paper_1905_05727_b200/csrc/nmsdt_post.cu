@@ -7,6 +7,7 @@
 // All sums have a fixed shape (no floating-point atomics): results are bit-identical from run to run.
 // These passes read the state once (56 B/cell) and are not part of sim_step; with the fused path's own elementary
 // functions (nmsdt_fast.cuh) the primitive recovery is cheap enough for them to be bound by HBM.
+#include <mutex>
 #include "nmsdt_host.h"
 #include "nmsdt_fast.cuh"
 
@@ -237,6 +238,78 @@ int launch_kinematics(const double* d_t, const double* d_xs, int n, double dtau,
 {
     k_kinematics<<<(n + 127) / 128, 128, 0, s>>>(d_t, d_xs, n, dtau, d_us, d_as);
     return 1;
+}
+
+} // namespace nmsdt
+
+// ---------------------------------------------------------------------------------------------------------------
+// sim_qdot_pdf_noalloc: the Eq. 14-16 histogram with its scratch in the library image instead of on the heap.
+//
+// Who needs it.  sim_qdot_pdf grows a per-handle scratch buffer with cudaMalloc / cudaFree on demand.  That is no use to
+// a host program that has handed every byte of the GPU to its own arena (a solver that lends this library its workspace
+// through sim_create's device_buf and has nothing left over for the driver's heap; cudaMalloc then fails although the
+// arena has room), nor to an in-situ monitor that samples the histogram every few steps next to sim_step calls queued
+// on other streams: cudaMalloc and cudaFree synchronise the whole device and would drain those queues at every sample.
+// For them the scratch is the fixed array below: it is part of libnmsdt.so's device image, so EVERY GPU on which the
+// library's kernels are loaded carries these ~2.3 MiB from that moment until the process exits, whether or not this entry
+// point is ever called.  That is why the limit is modest: POST_NOALLOC_MAX_BINS = 512 bins (the paper's window, P:317,
+// has 400); wider windows go through sim_qdot_pdf.
+//
+// Layout of the array (doubles): [0, nbins) mass, [nbins, 2 nbins) counts as unsigned 64-bit, then one row of nbins
+// partial masses per block of k_qdot_hist -- the layout launch_qdot_hist gives its heap buffer.
+// ---------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_noalloc_hist_scratch[(size_t)nmsdt::POST_HIST_BLOCKS * nmsdt::POST_NOALLOC_MAX_BINS +
+                                                                2 * (size_t)nmsdt::POST_NOALLOC_MAX_BINS];
+
+namespace nmsdt {
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+double* g_noalloc_addr[NOALLOC_MAX_DEVICES] = {};      // device address of the array on each ordinal, 0 = not looked up yet
+}
+
+// Returns the number of kernels enqueued, or -1 (argument) / -2 (CUDA) with *why pointing at a static message.
+// In host code `g_noalloc_hist_scratch` is only the handle the runtime registered for the symbol: its device address
+// differs per GPU and has to be asked for, once per device and with that device current (the first call on a device
+// does it here, under a lock; it also raises the dynamic shared-memory limit of k_qdot_hist on that device).
+int launch_qdot_hist_noalloc(const Params& P, const double* q, double n_lo, double dn, int nbins, double** d_mass, unsigned long long** d_count,
+                             cudaStream_t s, const char** why)
+{
+    if (nbins < 1 || nbins > POST_NOALLOC_MAX_BINS) { *why = "nbins outside [1, 512]: the static scratch holds 512 bins, use sim_qdot_pdf for more"; return -1; }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { *why = cudaGetErrorString(e); cudaGetLastError(); return -2; }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) { *why = "device ordinal beyond the 64 this entry point keeps addresses for"; return -1; }
+    cudaPointerAttributes at;
+    e = cudaPointerGetAttributes(&at, q);
+    if (e != cudaSuccess) { *why = cudaGetErrorString(e); cudaGetLastError(); return -2; }
+    if (at.type != cudaMemoryTypeDevice || at.device != dev) { *why = "the device that holds the handle's state must be the current device"; return -1; }
+    double* buf = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_addr[dev]) {
+            void* p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_noalloc_hist_scratch);
+            if (e != cudaSuccess || !p) { *why = e != cudaSuccess ? cudaGetErrorString(e) : "cudaGetSymbolAddress returned NULL"; cudaGetLastError(); return -2; }
+            e = cudaFuncSetAttribute(k_qdot_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(HW * POST_MAX_BINS * 12));
+            if (e != cudaSuccess) { *why = cudaGetErrorString(e); cudaGetLastError(); return -2; }
+            g_noalloc_addr[dev] = static_cast<double*>(p);
+        }
+        buf = g_noalloc_addr[dev];
+    }
+    double* mass = buf;
+    unsigned long long* count = reinterpret_cast<unsigned long long*>(buf + nbins);
+    double* part = buf + 2 * (size_t)nbins;
+    const size_t smem = (size_t)HW * nbins * (sizeof(double) + sizeof(int));
+    // The array keeps whatever the previous call (of any handle, any window) left in it.  Only the counts are accumulated
+    // (integer atomics) and must start at zero; every block overwrites its whole row of partial masses and k_hist_final
+    // overwrites the nbins masses, so nothing else of the old contents is ever read.
+    cudaMemsetAsync(count, 0, sizeof(unsigned long long) * nbins, s);
+    k_qdot_hist<<<POST_HIST_BLOCKS, HT, smem, s>>>(P, q, n_lo, dn, nbins, part, count);
+    k_hist_final<<<(nbins + 255) / 256, 256, 0, s>>>(part, POST_HIST_BLOCKS, nbins, mass);
+    *d_mass = mass; *d_count = count;
+    return 2;
 }
 
 } // namespace nmsdt
