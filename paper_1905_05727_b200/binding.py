@@ -157,10 +157,6 @@ def _dp(a):
 
 
 def workspace_bytes(grid):
-    return int(load_library().sim_workspace_bytes(C.byref(_fill(Grid(), grid))))
-
-
-def workspace_bytes(grid):
     """sim_workspace_bytes for a grid dict"""
     return int(load_library().sim_workspace_bytes(C.byref(_fill(Grid(), grid))))
 
