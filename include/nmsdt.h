@@ -71,7 +71,7 @@ typedef struct {
 /* Table III.  RK4 sub-stepping rule R13: n_sub = min(max_substeps, 1 + floor(theta/substep_theta)) */
 typedef struct {
     double Ta, Cpre, Q;
-    int reactive;               /* 0: inert (source step skipped) */
+    int reactive;               /* 0: inert (source step skipped); 1 needs Q, Cpre, Ta and eos cv2 > 0 (SIM_ERR_ARG otherwise) */
     int max_substeps;
     double substep_theta;
 } sim_kin_t;

@@ -347,6 +347,10 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     if (!(e->z_min > 0.0 && e->z_min < 0.5) || !(e->gamma1 > 1.0) || !(e->Gamma2 > 0.0) || !(e->rho02 > 0.0) || e->C == 1.0 || e->D == 1.0)
         return fail(nullptr, SIM_ERR_ARG, "sim_create: bad EOS parameters");
     if (k->max_substeps < 1 || !(k->substep_theta > 0.0)) return fail(nullptr, SIM_ERR_ARG, "sim_create: bad kinetics parameters");
+    // the fused source step decides all four RK4 stages by one T2 > 0 test (rk4_step, nmsdt_fast.cuh): that is the oracle's per-stage
+    // test only for an exothermic, forward reaction (beta = Q/cv2 > 0, C > 0, Ta > 0; Table II-III), so nothing else is taken
+    if (k->reactive && (!(k->Q > 0.0) || !(e->cv2 > 0.0) || !(k->Cpre > 0.0) || !(k->Ta > 0.0)))
+        return fail(nullptr, SIM_ERR_ARG, "sim_create: a reactive run needs Q > 0, cv2 > 0, Cpre > 0 and Ta > 0");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();

@@ -64,3 +64,27 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "oracle_py" not in src and "nmsdt_oracle" not in src and "liboracle" not in src, f
+
+
+def test_sim_create_rejects_reactive_runs_that_are_not_exothermic_forward_reactions(lib):
+    """rk4_step (nmsdt_fast.cuh) tests T2 > 0 once per RK4 step; that equals the oracle's per-stage test (O5) only for
+    Q/cv2 > 0, C > 0, Ta > 0 (Table II-III).  sim_create checks its arguments before it looks for a device, so
+    this runs on the CPU box."""
+    from paper_1905_05727_b200 import binding, inputs
+    c = inputs.config("C1", reactive=1)
+    g = binding._fill(binding.Grid(), c["grid"])
+    for kin_bad, eos_bad in ((dict(Q=0.0), {}), (dict(Q=-4.46e6), {}), (dict(Cpre=0.0), {}), (dict(Ta=-1.0), {}), ({}, dict(cv2=0.0)),
+                             (dict(Q=float("nan")), {})):
+        e = binding._fill(binding.Eos(), dict(c["eos"], **eos_bad))
+        k = binding._fill(binding.Kin(), dict(c["kin"], **kin_bad))
+        h = C.c_void_p()
+        assert lib.sim_create(C.byref(g), C.byref(e), C.byref(k), None, 0, None, C.byref(h)) == binding.SIM_ERR_ARG
+        assert b"reactive run needs" in lib.sim_last_error(None) and not h.value
+    # the same numbers are fine for an inert run: the argument check passes and the call gets as far as the device
+    e = binding._fill(binding.Eos(), c["eos"])
+    k = binding._fill(binding.Kin(), dict(c["kin"], Q=0.0, reactive=0))
+    h = C.c_void_p()
+    rc = lib.sim_create(C.byref(g), C.byref(e), C.byref(k), None, 0, None, C.byref(h))
+    assert rc in (binding.SIM_OK, binding.SIM_ERR_CUDA)
+    if rc == binding.SIM_OK:
+        lib.sim_destroy(h)
