@@ -102,7 +102,9 @@ size_t sim_workspace_bytes(const sim_grid_t* grid);
 
 /* Create a simulation. device_buf: DEVICE pointer to >= sim_workspace_bytes() bytes, 256-byte aligned, lent by
    the caller for the lifetime of the handle (e.g. a torch tensor), or NULL to let the library cudaMalloc it.
-   cuda_stream: a cudaStream_t (NULL = default stream). [sync] */
+   cuda_stream: a cudaStream_t (NULL = default stream). [sync]
+   If the driver cannot encode the tensor maps of the fused y-sweep (cuTensorMapEncodeTiled), the handle is still created, starts on
+   SIM_VARIANT_UNFUSED, says so in sim_last_error(handle), and sim_set_variant(SIM_VARIANT_FUSED) returns SIM_ERR_CUDA. */
 int sim_create(const sim_grid_t* grid, const sim_eos_t* eos, const sim_kin_t* kin,
                void* device_buf, size_t bytes, void* cuda_stream, sim_t** out);
 void sim_destroy(sim_t*);
@@ -241,8 +243,8 @@ int sim_set_variant(sim_t*, int variant, int use_graph);
 /* How sim_step enqueues the fused variant's kernels (2 per step: pass 1 and pass 2; ghost cells are taken from the
    boundary rule as the sweeps load them and the last block of pass 2 ends the step, so there is no halo or control
    launch): use_graph = pairs of steps replayed as one CUDA graph (default on), use_pdl = the kernels chained by
-   programmatic dependent launch, a kernel's prologue overlapping its predecessor's tail (default off: measured 3-6 %
-   slower than plain graph edges on the launch-bound configs, equal on the large ones).  They change when
+   programmatic dependent launch, a kernel's prologue overlapping its predecessor's tail (default off: on this two-launch
+   step it measures equal on the smallest and the largest grids and 3 % slower on the 4096 x 512 one).  They change when
    kernels start, never what they compute. */
 int sim_set_launch_mode(sim_t*, int use_graph, int use_pdl);
 /* Launch geometry of the fused sweep in direction dir (0 = x, 1 = y) on this grid: a block (y: 256 columns, x: 4 rows)

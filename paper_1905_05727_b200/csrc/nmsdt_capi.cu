@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -78,6 +79,7 @@ struct sim {
     double dt_mode = -1.0;          // dt_fixed the control block was last prepared for
     long long launches = 0;
     std::string err;
+    bool tm_ok = true;              // false: the tensor maps could not be encoded, the handle is confined to the unfused variant
     CUtensorMap tmA, tmB;           // the two plane sets as {pitch, rows, 7} tensors with a {32, 1, 7} box (y-sweep staging)
     sim_slab_peer_t peer[2];        // slab decomposition: connected neighbours (peer-store transport)
     bool peer_on[2] = {false, false};
@@ -203,15 +205,14 @@ bool make_plane_tensor_map(CUtensorMap* tm, const double* plane0, int pitch, int
     typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
     static encode_fn encode = nullptr;
-    if (!encode) {
+    static std::once_flag once;                      // handles may be created from several host threads at once
+    std::call_once(once, [] {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn) {
-            cudaGetLastError();
-            return false;
-        }
-        encode = (encode_fn)fn;
-    }
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess && fn) encode = (encode_fn)fn;
+        else cudaGetLastError();
+    });
+    if (!encode) return false;
     const cuuint64_t dims[3] = {(cuuint64_t)pitch, (cuuint64_t)rows, 7};
     const cuuint64_t strides[2] = {(cuuint64_t)pitch * sizeof(double), (cuuint64_t)fstride * sizeof(double)};     // bytes, dims 1 and 2
     const cuuint32_t box[3] = {32, 1, 7}, estr[3] = {1, 1, 1};
@@ -375,9 +376,11 @@ int sim_create(const sim_grid_t* g, const sim_eos_t* e, const sim_kin_t* k, void
     s->tab = (double*)(s->base + s->L.off_tab);
     fill_params(s);
     if (!make_plane_tensor_map(&s->tmA, s->A, s->L.pitch, s->L.rows, s->L.fstride) || !make_plane_tensor_map(&s->tmB, s->B, s->L.pitch, s->L.rows, s->L.fstride)) {
-        if (s->owns) cudaFree(s->base);
-        delete s;
-        return fail(nullptr, SIM_ERR_CUDA, "sim_create: cuTensorMapEncodeTiled failed (the y-sweep stages its rows with bulk tensor copies)");
+        // only the fused y-sweep stages its rows with bulk tensor copies: the unfused kernels, the x-only piecewise calls, diagnostics
+        // and post-processing do without.  The handle starts on the unfused variant and sim_set_variant refuses the fused one.
+        s->tm_ok = false;
+        s->variant = SIM_VARIANT_UNFUSED;
+        s->err = "sim_create: cuTensorMapEncodeTiled is unavailable or failed; this handle runs SIM_VARIANT_UNFUSED only";
     }
     init_fused_kernels();
     cudaMemsetAsync(s->base, 0, s->L.total, s->stream);
@@ -643,6 +646,8 @@ int sim_redo_count(sim_t* s, long long* n)
 int sim_set_variant(sim_t* s, int variant, int use_graph)
 {
     if (!s || (variant != SIM_VARIANT_UNFUSED && variant != SIM_VARIANT_FUSED)) return fail(s, SIM_ERR_ARG, "sim_set_variant: bad argument");
+    if (variant == SIM_VARIANT_FUSED && !s->tm_ok)
+        return fail(s, SIM_ERR_CUDA, "sim_set_variant: the fused variant needs tensor maps (cuTensorMapEncodeTiled failed in sim_create); this handle runs SIM_VARIANT_UNFUSED only");
     s->variant = variant; s->use_graph = use_graph ? 1 : 0; s->cfl_valid = false;
     return SIM_OK;
 }

@@ -4,8 +4,8 @@
 //   pass 1 = S(dt/2) applied on load + directional sweep d1          (k_xsweep<LEAD> or k_ysweep<LEAD>)
 //   pass 2 = directional sweep d2 + S(dt/2) on the updated cell + max-wavespeed partial of the new state
 //                                                                     (k_xsweep<TRAIL> or k_ysweep<TRAIL>)
-// followed by the one-thread k_ctl (t += dt, next CFL dt).  Algorithmic HBM traffic: 2 x (7 read + 7 written) planes
-// = 224 B per cell-step.  The arithmetic is that of nmsdt_device.cuh (O3-O5) with the branch-free elementary
+// and the block of pass 2 that finishes last ends the step (t += dt, next CFL dt: step_end_by_last_block; the one-thread k_ctl
+// is launched only by the piecewise slab calls).  Algorithmic HBM traffic: 2 x (7 read + 7 written) planes = 224 B per cell-step.  The arithmetic is that of nmsdt_device.cuh (O3-O5) with the branch-free elementary
 // functions of nmsdt_math.cuh; a warp whose segment holds a cell that needs one of the rare rules (RK4 sub-steps R13,
 // first-order fallback R17, a density outside the power tables) repeats the segment with the exact rules.
 //
@@ -198,6 +198,17 @@ __device__ __forceinline__ void trail_cell(const Params& P, const double* __rest
     const double a = dmax_(fabs(W.un), fabs(W.ut)) + q_sqrt(W.rc2 * W.irho);
     bad |= state_ok(o, a) ? 0 : 1;
     smax = dmax_(smax, a);
+}
+
+// dt and tsafe of the running step.  They live in the control block that the LAST block of this very kernel rewrites for the
+// next step (step_end_by_last_block) -- after every block has read them, the ticket sees to that -- so for the kernel as a whole
+// the two words are neither read-only nor unaliased: no __restrict__ / LDG.NC on them and no load the compiler may repeat later,
+// but exactly one L2 load per call of a segment function (the redo call reads the same, still unchanged, values again).
+__device__ __forceinline__ double ld_ctl(const double* p)
+{
+    double v;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
 }
 
 __device__ __forceinline__ void reduce_smax(double smax, int bad, Ctl* ctl)
@@ -396,7 +407,7 @@ struct YPipe { int st, ph; };
 // sub-stepping or the first-order fallback (EXACT = false only; the caller then redoes the segment with EXACT = true --
 // the pass is out of place).
 template <int MODE, bool EXACT, int LIM>
-__device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ qout, const double* __restrict__ dtp, int seg, int col, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad,
+__device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ qout, const double* dtp, int seg, int col, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad,
                                           const CUtensorMap* tm, unsigned bars, unsigned wmask, YPipe& pp)
 {
     // staged input rows: per warp YST stages of [7 planes][32 columns], each filled by one bulk tensor copy;
@@ -411,7 +422,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
     const int tid = threadIdx.x;
     bool hot = false;               // a cell needs the exact rules (R13 sub-steps or the R17 fallback): redo the segment
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.ny);
-    const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
+    const double dt = ld_ctl(dtp), tau = 0.5 * dt, Tsafe = ld_ctl(dtp + 1);
     const double dtdx = dt / P.dy, khalf = 0.5 * dtdx;
     // (the plane stride as a 32-bit number -- sim_create refuses planes of 2^32 doubles -- so that a plane's address is ONE
     // IMAD.WIDE.U32 from the row pointer instead of a 64 x 64-bit product)
@@ -536,7 +547,7 @@ __device__ __forceinline__ bool y_segment(const Params& P, double* __restrict__ 
 
 template <int MODE, int LIM>
 __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_constant__ Params P, const __grid_constant__ CUtensorMap tm,
-                                                                  double* __restrict__ qout, const double* __restrict__ dtp, Ctl* ctl, int seg, int end_step)
+                                                                  double* __restrict__ qout, const double* dtp, Ctl* ctl, int seg, int end_step)
 {
     extern __shared__ __align__(16) double s_dyn_raw[];
     // the staged rows are bulk-copy destinations and must be 128-byte aligned: the dynamic part follows the static arrays
@@ -576,7 +587,7 @@ __global__ void __launch_bounds__(YT, NMSDT_Y_MINBLOCKS) k_ysweep(const __grid_c
 // sub-stepping or the first-order fallback (EXACT = false only; the caller then redoes the segment with EXACT = true --
 // the pass is out of place).
 template <int MODE, bool EXACT, int LIM>
-__device__ __forceinline__ bool x_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* __restrict__ dtp,
+__device__ __forceinline__ bool x_segment(const Params& P, const double* __restrict__ qin, double* __restrict__ qout, const double* dtp,
                                           int seg, int row, const double* __restrict__ s_tab, double* __restrict__ s_dyn, double& smax, int& bad)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -590,7 +601,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
     double2* rf = rfr + 6 * RING;                    // [4][33]: flux of face A-1/2
     double2* stg = reinterpret_cast<double2*>(s_dyn + XW * RING_DOUBLES) + warp * 7 * PRING;   // [7][66] input pairs
     const int c0 = blockIdx.y * seg, c1 = min(c0 + seg, P.nx);
-    const double dt = dtp[0], tau = 0.5 * dt, Tsafe = dtp[1];
+    const double dt = ld_ctl(dtp), tau = 0.5 * dt, Tsafe = ld_ctl(dtp + 1);
     const double dtdx = dt / P.dx, khalf = 0.5 * dtdx;
     const unsigned long long fs = (unsigned)P.fstride;     // (32-bit plane stride: see y_segment)
     const unsigned long long fsb = fs * sizeof(double);
@@ -766,7 +777,7 @@ __device__ __forceinline__ bool x_segment(const Params& P, const double* __restr
 
 template <int MODE, int LIM>
 __global__ void __launch_bounds__(32 * XW, NMSDT_X_MINBLOCKS) k_xsweep(const __grid_constant__ Params P, const double* __restrict__ qin, double* __restrict__ qout,
-                                                    const double* __restrict__ dtp, Ctl* ctl, int seg, int end_step)
+                                                    const double* dtp, Ctl* ctl, int seg, int end_step)
 {
     extern __shared__ __align__(16) double s_dyn[];
     __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES];
@@ -821,8 +832,11 @@ __global__ void __launch_bounds__(128) k_source_fast(const __grid_constant__ Par
 //   * B > nsm * maxb (large grids): ceil(B / (nsm maxb)) waves of (seg + ramp + start) iterations, each at the throughput-bound
 //     pace of maxb resident blocks -- large grids end up near `target`, with little ramp-up redundancy;
 //   * otherwise one wave with b = ceil(B / nsm) blocks per SM, whose iterations take max(lat, b) / maxb of that pace: a lone
-//     block is bound by the latency of the cell's dependency chain (measured: an iteration of a lone block takes lat = 2.6 (y),
-//     2.5 (x) times as long as its share of a full SM's), so small grids are cut into as many short segments as the SMs
+//     block is bound by the latency of the cell's dependency chain (measured in round 1 with 4 resident blocks per SM in both
+//     directions: an iteration of a lone block took 2.6 (y, 128 columns) and 2.5 (x) times as long as its share of a full SM's.
+//     The unit of `lat` is one block's share, 1/maxb of the SM: the y-sweep now runs 256-column blocks, 2 per SM -- a lone one
+//     has twice the warps in flight and the same latency-bound iteration time, which is 2.6 x 2/4 = 1.3 of ITS share; that is
+//     the 1.3 launch_sweep_fused passes, rescaled, not measured again), so small grids are cut into as many short segments as the SMs
 //     can take before throughput binds -- on a machine that is not full, recomputed ramp-up cells are free and latency counts
 //     (C1: 6 instead of 12 rows per block).
 static double seg_cost(long long B, double iters, int nsm, int maxb, double lat)
