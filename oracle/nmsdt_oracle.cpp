@@ -390,6 +390,14 @@ extern "C" int orc_init_fields(orc_t* s, const double* const q[7])
     for (int f = 0; f < 7; ++f)
         for (int j = 0; j < s->g.ny; ++j)
             for (int i = 0; i < s->g.nx; ++i) s->q[f][s->idx(i, j)] = q[f][(size_t)j * s->g.nx + i];
+    /* R27: the stored volume fraction of every state the scheme holds lies in [z_min, 1 - z_min] -- O7 paints it
+       there, O4.6 clamps each update, O3 clamps at each primitive recovery -- so a caller's state is brought to the same
+       invariant on entry; otherwise O4.6 would use the raw value in the z1 (u* difference) term of the first sweep only. */
+    for (int j = 0; j < s->g.ny; ++j)
+        for (int i = 0; i < s->g.nx; ++i) {
+            double& z = s->q[5][s->idx(i, j)];
+            z = clampd(z, s->e.z_min, 1.0 - s->e.z_min);
+        }
     s->cav.clear();
     finish_init(s);
     return 0;

@@ -92,6 +92,37 @@ def test_generator_matches_oracle_at_full_c4_and_c5_sizes(O, B):
             assert 8000 < len(ref) < 13000
 
 
+def test_out_of_range_volume_fraction_is_clamped_on_entry_by_both_sides(O, B):
+    """R27: sim_init_fields and orc_init_fields both store q5 clamped to [z_min, 1 - z_min]; a buffer with q5 outside (0, 1,
+    beyond) gives the same stored state and the same first step on both sides, in both variants."""
+    cfg, o0 = _developed_c1(O, reactive=1, steps=200)
+    q = [a.copy() for a in o0.state()]
+    rng = np.random.default_rng(5)
+    zmin = cfg["eos"]["z_min"]
+    # out-of-range values only where the clamp returns (nearly) the value the developed state holds, so that the clamped
+    # state is a state of the scheme: pure liquid (q5 = z_min) -> 0, negative, 1e-9; cavity interior (q5 >= 1 - 2 z_min) -> 1, 1.2
+    lo, hi = np.flatnonzero(q[5].ravel() == zmin), np.flatnonzero(q[5].ravel() >= 1.0 - 2.0 * zmin)
+    assert lo.size > 1000
+    pick = rng.choice(lo, 300, replace=False)
+    q[5].ravel()[pick] = rng.choice([0.0, -0.1, 1e-9], 300)
+    if hi.size:
+        q[5].ravel()[hi] = rng.choice([1.0, 1.2, 1.0 - 1e-9], hi.size)
+    for variant in VARIANTS:
+        o, s = _pair(O, B, cfg, variant=variant)
+        o.init_fields(q)
+        s.init_fields(q)
+        for a, b in zip(s.state(), o.state()):
+            assert np.array_equal(a, b)
+        assert s.state()[5].min() == zmin and s.state()[5].max() <= 1.0 - zmin
+        assert np.array_equal(s.state()[5].ravel()[pick], np.full(300, zmin))
+        dt = o.cfl_dt()
+        assert s.cfl_dt() == pytest.approx(dt, rel=1e-13)
+        o.step_dt(1, 0.25 * dt)
+        s.step_dt(1, 0.25 * dt)
+        _assert_one_step(o, s, what="clamped entry state, variant %d" % variant)
+        s.close()
+
+
 # ------------------------------------------------------------------------------------------------ pieces
 def _developed_c1(O, reactive, steps=120, threads=8):
     cfg = inputs.config("C1", reactive=reactive)

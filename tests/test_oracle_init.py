@@ -124,3 +124,21 @@ def test_lattice_and_periodic_painting(O):
     o2.init(ini)
     z2 = o2.read_field("q5")
     assert z2[0, 31] > 0.999 and z2[63, 31] == 1e-6
+
+
+def test_init_fields_clamps_the_volume_fraction(O):
+    """R27: an explicit initial state is stored with q5 in [z_min, 1 - z_min] (the invariant O7 / O4.6 / O3 keep for every
+    state of the scheme); values inside are stored bit for bit, the other six fields are never touched."""
+    cfg = inputs.config("C2", nx=8, ny=4, reactive=0)
+    zmin = cfg["eos"]["z_min"]
+    o = O.Oracle(cfg["grid"], cfg["eos"], cfg["kin"])
+    o.init(dict(cfg["init"], shock_cells=2))
+    q = [a.copy() for a in o.state()]
+    q[5][0, :] = [0.0, -0.25, 1.0, 1.5, zmin, 1.0 - zmin, 0.5 * zmin, 0.3]
+    keep = [a.copy() for a in q]
+    o.init_fields(q)
+    got = o.state()
+    assert np.array_equal(got[5][0], [zmin, zmin, 1.0 - zmin, 1.0 - zmin, zmin, 1.0 - zmin, zmin, 0.3])
+    assert np.array_equal(got[5][1:], keep[5][1:])
+    for k in (0, 1, 2, 3, 4, 6):
+        assert np.array_equal(got[k], keep[k])
