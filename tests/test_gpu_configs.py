@@ -5,8 +5,9 @@ global-reaction-rate curve (Eq. 12-13) and overtake time within 0.5 %
   C1  256 x 128, 200 steps (+ 500)                       tests/test_gpu_parity.py
   C2  4096 x 32 at 8, 9.4 and 11 GPa, each run until the global reaction rate has peaked       here
   C3  4096 x 512, 500 steps                               here
-  C4  8192 x 1024: 1 step on the full grid in tests/test_gpu_parity.py (sampled windows); here a 1024 x 256 crop with the
-      same generator parameters through cavity collapse and hot-spot ignition, diagnostics every 10 steps
+  C4  8192 x 1024: here the full grid for 500 steps at 8 GPa; a 2048 x 512 crop at each of the config's three input
+      pressures (7, 8, 9 GPa); a 1024 x 256 crop at 9 GPa through cavity collapse and hot-spot ignition with diagnostics
+      every 10 steps (1 step on the full grid on sampled windows: tests/test_gpu_parity.py)
   C5  32768 x 4096: 1 step on the full grid in tests/test_gpu_parity.py; here the 4096 x 1024 crop SURVEY 8(d) names
       (6.7e10 oracle cell-updates for the full grid are out of reach), 500 steps
 
@@ -181,6 +182,63 @@ def test_c4_crop_cavity_collapse_rate_curve(O, B):
     assert max(l1) <= 10 * TOL_L1_500, l1
     _one_step_from(O, B, cfg, o, "C4 crop after %d steps" % nsteps, variants=(0, 1))
     print("C4 crop: rate %.3e -> %.3e /s, final L1 %.2e, T2max %.0f K" % (rb[k_before], rb[-1], max(l1), T2.max()))
+
+
+@pytest.mark.parametrize("p_shock", [7e9, 8e9, 9e9])
+def test_c4_one_step_and_early_run_at_each_input_pressure(O, B, p_shock):
+    """BASELINE config 4's three input shock pressures, 7 / 8 / 9 GPa (the random-cavity rate curves), on a
+    2048 x 512 crop with the config's generator parameters: one step on the initial state (both variants), 60 steps of
+    free running (own device-side CFL steps), one even and one odd step on the developed state"""
+    cfg = inputs.config("C4", nx=2048, ny=512, p_shock=p_shock)
+    o, s = _start(O, B, cfg)
+    assert len(o.cavities()) > 20
+    s0 = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"], variant=0)
+    s0.init_fields(o.state())
+    o.step(1), s.step(1), s0.step(1)
+    c = o.read_field("c")
+    for h in (s, s0):
+        r = rel_diff(h.state(), o.state(), c)
+        assert max(r) <= TOL_ONE_STEP, (p_shock, r)
+    s0.close()
+    o.step(59), s.step(59)
+    da, db = s.diagnostics(), o.diagnostics()
+    assert da["step"] == db["step"] == 60 and da["bad_state"] == 0
+    assert da["t"] == pytest.approx(db["t"], rel=1e-11)
+    assert da["M2r"] == pytest.approx(db["M2r"], rel=1e-11)
+    l1 = l1_rel(s.state(), o.state())
+    assert max(l1) <= TOL_L1_500, l1
+    # the shocked slab sits at the input pressure (the three runs really differ)
+    assert o.read_field("p")[:, :60].mean() == pytest.approx(p_shock, rel=2e-2)
+    _one_step_from(O, B, cfg, o, "C4 crop at %.0f GPa after 60 steps" % (p_shock / 1e9), variants=(0, 1))
+    s.close()
+
+
+@pytest.mark.slow
+def test_c4_full_size_500_steps(O, B):
+    """BASELINE config 4 at its own size, 8192 x 1024 with ~480 random cavities (phi = 3 %, d = 24 cells, seed 12345), 8 GPa:
+    cavity list bit-identical, one step <= 1e-11, 500 free-running steps L1 <= 1e-7 (north_star; SURVEY 8(d) "Parity workload").
+    4.2e9 oracle cell-updates: about 280 s on the 16 host threads of the GPU box, the longest test of the suite."""
+    cfg = inputs.config("C4")
+    o, s = _start(O, B, cfg)
+    s_gen = B.Sim(cfg["grid"], cfg["eos"], cfg["kin"])
+    s_gen.init(cfg["init"])
+    assert np.array_equal(s_gen.cavities(), o.cavities()) and 400 < len(o.cavities()) < 600
+    s_gen.close()
+    o.step(1), s.step(1)
+    r = rel_diff(s.state(), o.state(), o.read_field("c"))
+    assert max(r) <= TOL_ONE_STEP, r
+    o.step(499), s.step(499)
+    da, db = s.diagnostics(), o.diagnostics()
+    assert da["step"] == db["step"] == 500 and da["bad_state"] == 0
+    assert da["t"] == pytest.approx(db["t"], rel=1e-10)
+    l1 = l1_rel(s.state(), o.state())
+    assert max(l1) <= TOL_L1_500, l1
+    # integrals of two states that differ by L1 <= 1e-7 per field: 1e-9 (measured 1.2e-11 for M2r, the others closer)
+    for k in ("M2r", "mass1", "mass2", "momx", "energy"):
+        assert da[k] == pytest.approx(db[k], rel=1e-9), k
+    assert o.fallback_count() == 0 and s.redo_count() == 0
+    print("C4 full, 500 steps: L1 %s" % (["%.1e" % v for v in l1],))
+    s.close()
 
 
 # ------------------------------------------------------------------------------------------------ C5
