@@ -34,7 +34,7 @@ from paper_1905_05727_b200 import inputs  # noqa: E402
 METRIC = "fp64 cell-updates/s per 2D step"
 UNIT = "cell-updates/s"
 # the algorithmic FP64 work of one cell in one fused directional sweep comes from ncu's counters of the C5
-# launches, profiles/roofline_counts.json (written by paper_1905_05727_b200/roofline_counts.py, which also records a hash of
+# launches, profiles/roofline_counts.json (written by roofline_counts.py, which also records a hash of
 # the kernel sources): FP64-pipe instructions (every DADD/DMUL/DFMA/DSETP occupies the half-rate pipe for one issue slot),
 # flops with dadd = dmul = 1, dfma = 2, dsetp = 0, and the measured DRAM bytes per cell.
 FP64_LANES_PER_SM, N_SM = 64, 148
@@ -42,7 +42,7 @@ FP64_LANES_PER_SM, N_SM = 64, 148
 
 def load_counts():
     """(counts, stale): per-kernel per-cell counts of the last ncu capture; stale = the kernel sources changed since"""
-    from paper_1905_05727_b200 import roofline_counts
+    import roofline_counts
     with open(os.path.join(ROOT, "profiles", "roofline_counts.json")) as f:
         c = json.load(f)
     return c, roofline_counts.source_hash() != c["source_sha256"]

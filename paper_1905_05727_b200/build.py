@@ -10,8 +10,9 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnmsdt.so")
-SOURCES = ["nmsdt_step.cu", "nmsdt_fused.cu", "nmsdt_init.cu", "nmsdt_post.cu", "nmsdt_slab.cu", "nmsdt_capi.cu"]
-HEADERS = ["nmsdt_device.cuh", "nmsdt_math.cuh", "nmsdt_fast.cuh", "nmsdt_host.h", os.path.join("..", "..", "include", "nmsdt.h")]
+SOURCES = ["nmsdt_step.cu", "nmsdt_fused.cu", "nmsdt_init.cu", "nmsdt_post.cu", "nmsdt_slab.cu", "nmsdt_probe.cu", "nmsdt_capi.cu"]
+HEADERS = ["nmsdt_device.cuh", "nmsdt_math.cuh", "nmsdt_fast.cuh", "nmsdt_host.h", os.path.join("..", "..", "include", "nmsdt.h"),
+           os.path.join("..", "..", "include", "nmsdt_probe.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v"]
 
@@ -31,11 +32,10 @@ def build(force=False, verbose=False):
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     nvcc = _nvcc()
-    extra = os.environ.get("NMSDT_NVCC_EXTRA", "").split()      # e.g. "-DNMSDT_Y_MINBLOCKS=4" for tuning sweeps
 
     def compile_one(src):
         obj = os.path.join(objdir, os.path.basename(src).replace(".cu", ".o"))
-        r = subprocess.run([nvcc] + NVCC_FLAGS + extra + ["-c", src, "-o", obj], capture_output=True, text=True)
+        r = subprocess.run([nvcc] + NVCC_FLAGS + ["-c", src, "-o", obj], capture_output=True, text=True)
         with open(obj + ".log", "w") as f:
             f.write(r.stdout + r.stderr)
         if r.returncode != 0:

@@ -1,5 +1,6 @@
 // nmsdt_capi.cu -- the C ABI of libnmsdt.so (include/nmsdt.h): handle, workspace layout, step orchestration.
 #include "../../include/nmsdt.h"
+#include "../../include/nmsdt_probe.h"
 #include "nmsdt_host.h"
 #include "nmsdt_math.cuh"
 

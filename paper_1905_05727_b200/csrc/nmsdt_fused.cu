@@ -970,47 +970,4 @@ void launch_ctl(const Params& P, Ctl* ctl, int advance, cudaStream_t s, bool pdl
 
 double host_tsafe(double tau, double Cpre, double Ta, double theta0) { return tsafe_for(tau, Cpre, Ta, theta0); }
 
-// ---------------------------------------------------------------------------------------------------------------
-// sim_probe_math: evaluate the elementary functions of nmsdt_math.cuh on device arrays (accuracy tests)
-// ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_probe_math(const __grid_constant__ PowCoef pw, const double* __restrict__ tab_g, int fn, const double* __restrict__ x, int n, double a, double b,
-                                                    double* __restrict__ y0, double* __restrict__ y1)
-{
-    __shared__ __align__(16) double s_tab[MATH_TAB_DOUBLES_LOG];
-    for (int i = threadIdx.x; i < MATH_TAB_DOUBLES_LOG; i += blockDim.x) s_tab[i] = tab_g[i];
-    __syncthreads();
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double v = x[i];
-    double r0 = 0.0, r1 = 0.0;
-    switch (fn) {
-    case 0: r0 = q_rcp(v); break;
-    case 1: r0 = q_sqrt(v); break;
-    case 2: r0 = q_log(s_tab, v); break;
-    case 3: q_pow_pair(s_tab, v, a * LOG2E, b * LOG2E, r0, r1); break;      // (v^a, v^b)
-    case 4: r0 = q_exp_neg(s_tab, v); break;
-    case 5: r0 = floor1(v); r1 = clamp01(v); break;
-    case 6: r0 = nonneg(v); r1 = cap690(v); break;
-    case 8: r0 = q_sqrt_ratio_floor1(v, a); r1 = q_sqrt_ratio_floor1(a, v); break;   // max(sqrt(x/a), 1), max(sqrt(a/x), 1)
-    case 7: if (!q_pow_tab(s_tab, pw, v, r0, r1)) { r0 = pow(v, pw.C); r1 = pow(v, pw.D); } break;   // the step kernels' route for Eq. 3-4
-    default: break;
-    }
-    y0[i] = r0; y1[i] = r1;
-}
-
-int launch_probe_math(const PowCoef& pw, const double* tab_dev, int fn, const double* host_x, int n, double a, double b, double* host_y0, double* host_y1,
-                      cudaStream_t s)
-{
-    double *dx = nullptr, *dy = nullptr;
-    if (cudaMalloc(&dx, sizeof(double) * n) != cudaSuccess) return -2;
-    if (cudaMalloc(&dy, sizeof(double) * 2 * n) != cudaSuccess) { cudaFree(dx); return -2; }
-    cudaMemcpyAsync(dx, host_x, sizeof(double) * n, cudaMemcpyHostToDevice, s);
-    k_probe_math<<<(n + 127) / 128, 128, 0, s>>>(pw, tab_dev, fn, dx, n, a, b, dy, dy + n);
-    cudaMemcpyAsync(host_y0, dy, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
-    cudaMemcpyAsync(host_y1, dy + n, sizeof(double) * n, cudaMemcpyDeviceToHost, s);
-    const cudaError_t e = cudaStreamSynchronize(s);
-    cudaFree(dx); cudaFree(dy);
-    return e == cudaSuccess ? 0 : -2;
-}
-
 } // namespace nmsdt

@@ -238,114 +238,4 @@ void launch_advance(Ctl* ctl, cudaStream_t s) { k_advance<<<1, 1, 0, s>>>(ctl); 
 __global__ void k_set_double(double* p, double v) { *p = v; }
 void launch_set_double(double* p, double v, cudaStream_t s) { k_set_double<<<1, 1, 0, s>>>(p, v); }
 
-// ---------------------------------------------------------------------------------------------------------
-// FP64 FMA throughput probe: 8 independent DFMA chains per thread
-// ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_probe_fp64(double* out, int iters, double a, double b)
-{
-    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
-    for (int i = 0; i < iters; ++i) {
-        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
-    }
-    out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
-}
-
-int launch_probe_fp64(cudaStream_t s, double* gflops, double* ms_out)
-{
-    const int blocks = 148 * 8, threads = 256, iters = 1 << 14;
-    double* d = nullptr;
-    if (cudaMalloc(&d, sizeof(double) * blocks * threads) != cudaSuccess) return -2;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    k_probe_fp64<<<blocks, threads, 0, s>>>(d, 1024, 0.999999, 1e-9);   // warm-up
-    float best = 1e30f;
-    for (int r = 0; r < 5; ++r) {
-        cudaEventRecord(e0, s);
-        k_probe_fp64<<<blocks, threads, 0, s>>>(d, iters, 0.999999, 1e-9);
-        cudaEventRecord(e1, s);
-        cudaEventSynchronize(e1);
-        float ms; cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(d);
-    if (cudaGetLastError() != cudaSuccess) return -2;
-    const double flop = 2.0 * 8.0 * (double)iters * blocks * threads;
-    *gflops = flop / (best * 1e-3) * 1e-9;
-    *ms_out = best;
-    return 0;
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// Issue-slot probe: 8 independent DFMA chains per thread with M independent 32-bit ALU instructions (LOP3) interleaved per
-// 8 DFMA, at the sweeps' residency (4 warps per scheduler).  Answers whether the other half of the sweeps' instruction
-// stream can hide under the half-rate FP64 pipe: T(M)/T(0) = 1 for M <= 8 if a DFMA holds the scheduler's issue port for
-// one cycle, (16 + M)/16 if it holds it for the two cycles its 16 lanes are busy.
-// ---------------------------------------------------------------------------------------------------------
-template <int M>
-__global__ void __launch_bounds__(128) k_probe_issue(double* out, int iters, double a, double b, unsigned c)
-{
-    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
-    unsigned y[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) y[k] = threadIdx.x * 8 + k;
-    // (xor and add alternate on every chain so that no two consecutive instructions of a chain fold into one)
-    for (int i = 0; i < iters; i += 2) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-#pragma unroll
-            for (int r = 0; r < 8; ++r) {
-                double& x = r == 0 ? x0 : r == 1 ? x1 : r == 2 ? x2 : r == 3 ? x3 : r == 4 ? x4 : r == 5 ? x5 : r == 6 ? x6 : x7;
-                asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(x) : "d"(a), "d"(b));
-#pragma unroll
-                for (int m = 0; m < (M + 7 - r) / 8; ++m) {          // M / 8 each, the first M % 8 DFMA one more
-                    unsigned& yy = y[(r + 3 * m) & 7];
-                    if ((h + m) & 1) asm volatile("add.u32 %0, %0, %1;" : "+r"(yy) : "r"(c));
-                    else             asm volatile("xor.b32 %0, %0, %1;" : "+r"(yy) : "r"(c));
-                }
-            }
-        }
-    }
-    unsigned ys = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) ys ^= y[k];
-    out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7 + (double)ys;
-}
-
-template <int M>
-static float time_probe_issue(cudaStream_t s, double* d, int blocks, int iters, cudaEvent_t e0, cudaEvent_t e1)
-{
-    k_probe_issue<M><<<blocks, 128, 0, s>>>(d, 256, 0.999999, 1e-9, 0x5bd1e995u);      // warm-up
-    float best = 1e30f;
-    for (int r = 0; r < 3; ++r) {
-        cudaEventRecord(e0, s);
-        k_probe_issue<M><<<blocks, 128, 0, s>>>(d, iters, 0.999999, 1e-9, 0x5bd1e995u);
-        cudaEventRecord(e1, s);
-        cudaEventSynchronize(e1);
-        float ms; cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
-    }
-    return best;
-}
-
-// ms[k] = time of the probe with M = 0, 4, 8, 16 other instructions per 8 DFMA (4 blocks of 4 warps per SM, one wave)
-int launch_probe_issue(cudaStream_t s, double ms[4])
-{
-    int dev = 0, nsm = 148; cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    const int blocks = nsm * 4, iters = 1 << 13;
-    double* d = nullptr;
-    if (cudaMalloc(&d, sizeof(double) * blocks * 128) != cudaSuccess) return -2;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    ms[0] = time_probe_issue<0>(s, d, blocks, iters, e0, e1);
-    ms[1] = time_probe_issue<4>(s, d, blocks, iters, e0, e1);
-    ms[2] = time_probe_issue<8>(s, d, blocks, iters, e0, e1);
-    ms[3] = time_probe_issue<16>(s, d, blocks, iters, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(d);
-    return cudaGetLastError() == cudaSuccess ? 0 : -2;
-}
-
 } // namespace nmsdt

@@ -1,13 +1,17 @@
 """Seeded, synthetic workload recipes shared by the tests, bench.py and smoke().
 
-This module holds NONE of the method's arithmetic: only the constants the paper prints
+This module holds none of the method's arithmetic on fields: only the constants the paper prints
 (Tables I-III; ambient state P:141) and the grid / cavity-layout / boundary
 parameters of the five BASELINE.json configs.
 Both the CUDA library and the oracle turn these plain dicts into fields with their own code.
+One formula of the paper does appear: `paper_case` uses Eq. 7 (delta_c = sqrt(pi d_c^2 / 4 phi))
+to write the EXPLICIT cavity list of the regular array, which both sides then receive as a list;
+the oracle's own Eq. 7 is pinned apart from it (tests/test_oracle_init.py).
 
 The paper measures on no public dataset; these generated fields take the shapes of its three
 scenarios (neat NM, regular cavity array, hundreds of random cavities) and stand in
-for its production grids (24000x313, 24000x2000 at dx = 1 um), which are not run.
+for its production grids (24000x313, 24000x2000 at dx = 1 um; `paper_case`, config names
+'P313' / 'P2000' for bench.py), which the parity tests do not run.
 """
 import copy
 
@@ -34,10 +38,27 @@ def _grid(nx, ny, dx, bcx=(BC_TRANSMISSIVE, BC_TRANSMISSIVE), bcy=(BC_PERIODIC, 
 
 
 def config(name, p_shock=None, reactive=None, nx=None, ny=None, seed=None):
-    """Return dict(grid, eos, kin, init, steps, name) for BASELINE.json config 'C1'..'C5'.
+    """Return dict(grid, eos, kin, init, steps, name) for BASELINE.json config 'C1'..'C5', or for the paper's two production
+    grids 'P313' / 'P2000'.
 
     nx/ny override the grid size (a crop with the same generator parameters; the cavity
     region keeps its x_lo and is clipped to the new nx)."""
+    if name in ("P313", "P2000"):
+        # the paper's own production grids at dx = 1 um (P:411, P:425), as bench.py workloads: 24000 x 313 (regular array,
+        # phi = 8 %) and 24000 x 2000 (random cavities, phi = 5 %, seed 2019), 7.81 GPa; see paper_case
+        cfg = paper_case("regular" if name == "P313" else "random", 1.0, p_shock=7.81e9 if p_shock is None else p_shock,
+                         seed=2019 if seed is None else seed)
+        cfg["name"], cfg["steps"] = name, 200
+        if nx is not None:
+            cfg["grid"]["nx"] = int(nx)
+            cfg["init"]["x_hi"] = min(cfg["init"]["x_hi"], int(nx))
+            cfg["init"]["cavities"] = [c for c in cfg["init"].get("cavities", []) if c[0] + c[2] < nx]
+        if ny is not None:
+            cfg["grid"]["ny"] = int(ny)
+            cfg["init"]["cavities"] = [c for c in cfg["init"].get("cavities", []) if c[1] + c[2] < ny]
+        if reactive is not None:
+            cfg["kin"]["reactive"] = int(reactive)
+        return cfg
     eos, kin, init = copy.deepcopy(EOS), copy.deepcopy(KIN), copy.deepcopy(_INIT0)
     dx24 = 100e-6 / 24.0       # 24 cells per 100 um cavity diameter (DESIGN R21)
     if name == "C1":           # single cavity, 256x128, transmissive everywhere

@@ -8,7 +8,7 @@ smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,smsp__sass_thread_inst_execu
         python bench.py --steps 2 --warmup 3 --no-e2e --no-cpu --no-slab
     # here (no GPU needed):
     ncu -i gpurun_out/sweeps_c5.ncu-rep --page raw --csv > sweeps_c5_raw.csv
-    python -m paper_1905_05727_b200.roofline_counts sweeps_c5_raw.csv --nx 32768 --ny 4096 --seg-x 3644 --seg-y 256 \
+    python roofline_counts.py sweeps_c5_raw.csv --nx 32768 --ny 4096 --seg-x 3644 --seg-y 256 \
         --command "<the ncu command>" --out profiles/roofline_counts.json
 
 What is counted: warp instructions executed on the FP64 pipe (DADD, DMUL, DFMA, DSETP alike: each holds
@@ -23,7 +23,7 @@ import json
 import os
 import re
 
-HERE = os.path.dirname(os.path.abspath(__file__))
+HERE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_1905_05727_b200")
 # everything the sweep kernels are compiled from: a change to any of these files invalidates the counts
 SOURCES = ["csrc/nmsdt_fused.cu", "csrc/nmsdt_fast.cuh", "csrc/nmsdt_math.cuh", "csrc/nmsdt_device.cuh"]
 MODES = {1: "lead", 2: "trail", 0: "plain", 3: "trail_inert"}

@@ -18,9 +18,14 @@ def lib():
 
 def test_header_symbols_are_all_exported(lib):
     from paper_1905_05727_b200 import binding
-    hdr = open(os.path.join(ROOT, "include", "nmsdt.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(sim_[a-z0-9_]+)\s*\(", hdr))
+    declared = set()
+    for name in ("nmsdt.h", "nmsdt_probe.h"):
+        hdr = open(os.path.join(ROOT, "include", name)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        found = set(re.findall(r"\b(sim_[a-z0-9_]+)\s*\(", hdr))
+        # the method's header holds no probe, the probes' header nothing else
+        assert all(f.startswith("sim_probe_") == (name == "nmsdt_probe.h") for f in found), (name, found)
+        declared |= found
     assert declared == set(binding.SYMBOLS)
     for name in declared:
         assert getattr(lib, name) is not None

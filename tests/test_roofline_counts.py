@@ -1,10 +1,10 @@
 """The roofline block of bench.py is computed from ncu counts of the sweep kernels (profiles/roofline_counts.json).  The file
 carries a hash of the kernel sources: these tests fail when a kernel source was edited and the counts were not taken again
-(`python -m paper_1905_05727_b200.roofline_counts`, see its docstring), so `roofline.frac` cannot silently drift from the build."""
+(`python roofline_counts.py`, see its docstring), so `roofline.frac` cannot silently drift from the build."""
 import json
 import os
 
-from paper_1905_05727_b200 import roofline_counts
+import roofline_counts
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -18,7 +18,7 @@ def test_counts_belong_to_the_kernel_sources_in_the_tree():
     c = _counts()
     assert c["source_sha256"] == roofline_counts.source_hash(), (
         "kernel sources changed since the ncu capture behind profiles/roofline_counts.json: capture again and rerun "
-        "python -m paper_1905_05727_b200.roofline_counts")
+        "python roofline_counts.py")
     assert c["source_files"] == ["paper_1905_05727_b200/" + f for f in roofline_counts.SOURCES]
     assert c["ncu_command"].startswith("ncu ") and "bench.py" in c["ncu_command"]
 
